@@ -1,0 +1,482 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (no GPU needed).
+
+Each test names the pin (P0..P13 of DESIGN.md "Oracle pins") and the passage it fixes.  None of
+them re-types the oracle's own formula and compares it with itself: they use closed forms,
+invariants, exact discrete recurrences, symmetries, brute force with an independent formulation,
+library routines and published known-answer vectors.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _periodic_bc(orc, drag_vector=False):
+    return orc.bc_flags("periodic", "periodic", drag_vector)
+
+
+# ------------------------------------------------------------------------------------------
+# P0: lattice identities (tables, Eq. 3, Eq. 4)
+# ------------------------------------------------------------------------------------------
+
+def test_p0_lattice_isotropy(orc):
+    c, w, opp, mir = orc.tables()
+    assert c.shape == (19, 3) and len({tuple(v) for v in c}) == 19
+    assert np.all(np.abs(c).sum(1) <= 2) and np.all(np.abs(c).max(1) <= 1)
+    assert abs(w.sum() - 1) < 1e-15
+    assert np.allclose((w[:, None] * c).sum(0), 0, atol=1e-16)
+    second = np.einsum("i,ia,ib->ab", w, c, c)
+    assert np.allclose(second, np.eye(3) / 3, atol=1e-16)
+    third = np.einsum("i,ia,ib,ic->abc", w, c, c, c)
+    assert np.allclose(third, 0, atol=1e-16)
+    # fourth-order isotropy: sum w c_a c_b c_c c_d = cs^4 (d_ab d_cd + d_ac d_bd + d_ad d_bc)
+    d = np.eye(3)
+    iso4 = (np.einsum("ab,cd->abcd", d, d) + np.einsum("ac,bd->abcd", d, d)
+            + np.einsum("ad,bc->abcd", d, d)) / 9
+    assert np.allclose(np.einsum("i,ia,ib,ic,id->abcd", w, c, c, c, c), iso4, atol=1e-16)
+    # opposite and mirror maps
+    assert np.array_equal(c[opp], -c)
+    assert np.array_equal(c[mir], c * np.array([1, -1, 1]))
+    assert np.array_equal(opp[opp], np.arange(19)) and np.array_equal(mir[mir], np.arange(19))
+    assert np.allclose(w[opp], w) and np.allclose(w[mir], w)
+
+
+def test_p0_equilibrium_moments(orc):
+    c, w, _, _ = orc.tables()
+    rng = np.random.default_rng(1)
+    for _ in range(20):
+        rho = rng.uniform(0.9, 1.1)
+        u = rng.uniform(-0.1, 0.1, 3)
+        fe = orc.feq(rho, u)
+        assert abs(fe.sum() - rho) < 1e-15
+        assert np.allclose(fe @ c, rho * u, atol=1e-16)
+        Pi = np.einsum("i,ia,ib->ab", fe, c, c)
+        assert np.allclose(Pi, rho * np.eye(3) / 3 + rho * np.outer(u, u), atol=1e-16)
+    assert np.allclose(orc.feq(1.0, np.zeros(3)), w, atol=0)
+
+
+def test_p0_guo_moments(orc):
+    c, _, _, _ = orc.tables()
+    rng = np.random.default_rng(2)
+    for _ in range(20):
+        tau = rng.uniform(0.5005, 1.5)
+        u = rng.uniform(-0.1, 0.1, 3)
+        F = rng.uniform(-1e-3, 1e-3, 3)
+        Fi = orc.guo(tau, u, F)
+        pref = 1 - 1 / (2 * tau)
+        assert abs(Fi.sum()) < 1e-18
+        assert np.allclose(Fi @ c, pref * F, atol=1e-18)
+        P2 = np.einsum("i,ia,ib->ab", Fi, c, c)
+        assert np.allclose(P2, pref * (np.outer(u, F) + np.outer(F, u)), atol=1e-18)
+
+
+# ------------------------------------------------------------------------------------------
+# P7: tau_total (Eqs. 9-12, reading R9)
+# ------------------------------------------------------------------------------------------
+
+def test_p7_tau_total_self_consistency(orc):
+    """If Pi_neq = -(2/3) rho tau_t S with tau_t = tau0 + 3 C_smag |S|, |S| = sqrt(2 S:S)
+    (Eqs. 8-9 with nu = (tau - 1/2)/3), then Eq. 10 -> Eq. 12 must return that same tau_t."""
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        A = rng.normal(size=(3, 3)) * 10 ** rng.uniform(-5, -1)
+        S = 0.5 * (A + A.T)
+        S -= np.trace(S) / 3 * np.eye(3)
+        rho = rng.uniform(0.9, 1.1)
+        tau0 = 0.5 + 3 * 10 ** rng.uniform(-5, -1)
+        Csmag = rng.uniform(0.005, 0.03)
+        Smag = np.sqrt(2 * np.sum(S * S))
+        tau_t = tau0 + 3 * Csmag * Smag
+        Pn = -(2.0 / 3.0) * rho * tau_t * S
+        p6 = [Pn[0, 0], Pn[1, 1], Pn[2, 2], Pn[0, 1], Pn[1, 2], Pn[0, 2]]
+        got = orc.tau_total(tau0, Csmag, rho, p6)
+        assert abs(got - tau_t) < 1e-14 * tau_t
+    # limits: Cs = 0 or Q = 0 give tau0
+    assert orc.tau_total(0.5003, 0.0, 1.02, [1e-3, -2e-3, 1e-3, 4e-4, 0, 1e-4]) == pytest.approx(0.5003, abs=1e-16)
+    assert orc.tau_total(0.5003, 0.01, 1.02, [0] * 6) == pytest.approx(0.5003, abs=1e-16)
+    # off-diagonals count twice (":" is the full double contraction): xy-only vs xx-only tensors
+    t_xy = orc.tau_total(0.6, 0.01, 1.0, [0, 0, 0, 1e-3, 0, 0])
+    t_xx = orc.tau_total(0.6, 0.01, 1.0, [np.sqrt(2) * 1e-3, 0, 0, 0, 0, 0])
+    assert t_xy == pytest.approx(t_xx, rel=1e-15)
+
+
+def test_paper_table1_lattice_units(orc):
+    """Table I: Eq. 16 read as a force density reproduces Re_tau ~ 180, and
+    nu_lat = nu dt / dx^2 gives tau0 = 3 nu_lat + 1/2 = 0.500887 (readings R3, R4)."""
+    g = {}
+    for line in open(os.path.join(GOLD, "paper_table1.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        g[k] = float(v)
+    u_tau = np.sqrt(g["F"] * g["H"] / 1.0)
+    Re_tau = u_tau * g["H"] / g["nu"]
+    assert abs(Re_tau - g["Re_tau_nominal"]) / g["Re_tau_nominal"] < 0.02   # 177.6 vs 180
+    nu_lat = g["nu"] * g["dt"] / g["dx"] ** 2
+    o = orc.Oracle(4, 4, 4, nu_lat, np.sqrt(g["C_smag"]))
+    assert o.tau0 == pytest.approx(0.500887, abs=5e-7)
+    # paper-sized workload in workloads.PAPER_SIZED uses exactly these lattice values
+    pc = wl.get("paper_channel")
+    assert pc["nu"] == pytest.approx(nu_lat, rel=1e-12)
+    assert pc["body_force"][0] == pytest.approx(g["F"] * g["dt"] ** 2 / g["dx"], rel=1e-4)
+    assert (pc["nx"], pc["ny"], pc["nz"]) == (12 * 31, 2 * 31, 4 * 31)
+    # Table III: cell-count ratios the prose prints
+    assert 250 * 100 * 200 / g["coarse_cells"] == pytest.approx(g["medium_ratio"], abs=0.01)
+    assert 350 * 140 * 280 / g["coarse_cells"] == pytest.approx(g["fine_ratio"], abs=0.01)
+    assert round(20.0 / (1000.0 / 350.0)) == g["forest_cells_fine"]
+
+
+# ------------------------------------------------------------------------------------------
+# RNG and LAD table
+# ------------------------------------------------------------------------------------------
+
+def test_rng_known_answers(orc):
+    for line in open(os.path.join(GOLD, "splitmix64_vectors.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        seed, n, val = (int(t) for t in line.split())
+        assert orc.mix64(seed, n) == val
+        assert orc.rand01(seed, n) == (val >> 11) / 2.0 ** 53
+    r = np.array([orc.rand01(12345, i) for i in range(20000)])
+    assert 0 <= r.min() and r.max() < 1
+    assert abs(r.mean() - 0.5) < 0.01 and abs(r.var() - 1 / 12) < 0.003
+
+
+def test_lad_profile_closed_forms(orc):
+    from scipy.integrate import quad
+    # Eq. 14: maximum 1 at eta_m, both branches of Eq. 15 give 1 there
+    assert orc.lad_shape(0.7, 0.7) == pytest.approx(1.0, abs=1e-15)
+    assert orc.lad_shape(0.7 - 1e-12, 0.7) == pytest.approx(1.0, abs=1e-9)
+    eta = np.linspace(0, 0.999, 2000)
+    s = np.array([orc.lad_shape(e, 0.7) for e in eta])
+    assert s.max() <= 1.0 + 1e-15 and abs(eta[s.argmax()] - 0.7) < 1e-3
+    # s(0) = 0.3^6 e^{6 (1 - 0.3)} (n = 6 branch), s -> 0 as eta -> 1 (n = 1/2 branch)
+    assert orc.lad_shape(0.0, 0.7) == pytest.approx(0.3 ** 6 * np.exp(4.2), rel=1e-14)
+    assert orc.lad_shape(0.9999, 0.7) < 1e-10 and orc.lad_shape(1.0, 0.7) == 0.0
+    # upper branch n = 1/2 at eta = 0.85: r = 2, s = sqrt(2) exp(-1/2)
+    assert orc.lad_shape(0.85, 0.7) == pytest.approx(np.sqrt(2) * np.exp(-0.5), rel=1e-14)
+    integral, _ = quad(lambda e: orc.lad_shape(e, 0.7), 0, 1, points=[0.7], limit=200)
+    assert integral == pytest.approx(0.4601, abs=2e-4)
+    for h, ny in ((16, 128), (32, 256), (48, 384)):
+        a = orc.lad_profile(h, ny, 2.0, 0.7)
+        assert a.sum() == pytest.approx(2.0, rel=1e-14)          # LAI = sum a_j dy
+        assert np.all(a[h:] == 0) and np.all(a[:h] > 0)
+        j_peak = int(np.argmax(a))
+        assert abs((j_peak + 0.5) / h - 0.7) <= 0.5 / h + 1e-12   # one peak at 0.7 h
+        assert np.all(np.diff(a[: j_peak + 1]) > 0) and np.all(np.diff(a[j_peak:h]) < 0)
+        # midpoint rule converges to LAI / (h * integral) at the peak
+        assert a.max() == pytest.approx(2.0 / (h * 0.4601), rel=0.02)
+
+
+# ------------------------------------------------------------------------------------------
+# P1 rest state, P2 mass
+# ------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("bottom,top", [("bounce_back", "bounce_back"), ("bounce_back", "free_slip"),
+                                        ("periodic", "periodic")])
+def test_p1_rest_state(orc, bottom, top):
+    _, w, _, _ = orc.tables()
+    lad = np.zeros(10)
+    lad[:3] = 0.2
+    o = orc.Oracle(8, 10, 6, 1e-4, 0.1, (0, 0, 0), 0.2, lad, orc.bc_flags(bottom, top))
+    o.step(300)
+    f = o.get_populations()
+    assert np.max(np.abs(f - w[:, None, None, None])) < 1e-15
+    rho, u = o.get_macros()
+    assert np.max(np.abs(rho - 1)) < 1e-15 and np.max(np.abs(u)) < 1e-15
+
+
+def test_p2_mass_conservation(orc):
+    cfg = wl.small(16, 12, 8, nu=1e-4, Fx=3e-6)
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    m0 = o.get_macros()[0].sum()
+    f0 = o.get_populations().sum()
+    for _ in range(4):
+        o.step(250)
+        assert abs(o.get_macros()[0].sum() - m0) / m0 < 1e-12
+        assert abs(o.get_populations().sum() - f0) / f0 < 1e-12
+
+
+# ------------------------------------------------------------------------------------------
+# P3 Poiseuille, P4 Taylor-Green
+# ------------------------------------------------------------------------------------------
+
+def _poiseuille(orc, nu, top, ny=32, F=1e-6, efolds=8.0):
+    o = orc.Oracle(4, ny, 4, nu, 0.0, (F, 0, 0), 0.0, None, orc.bc_flags("bounce_back", top))
+    H = ny if top == "bounce_back" else 2 * ny
+    o.step(int(efolds * H * H / (np.pi ** 2 * nu)))     # slowest mode decays as exp(-pi^2 nu t / H^2)
+    rho, u = o.get_macros()
+    y = np.arange(ny) + 0.5
+    H = ny if top == "bounce_back" else 2 * ny
+    exact = F / (2 * nu) * y * (H - y)
+    ux = u[0].mean(axis=(0, 2))
+    assert np.max(np.abs(u[0] - ux[None, :, None])) < 1e-12 * exact.max()
+    assert np.max(np.abs(u[1])) < 1e-12 and np.max(np.abs(u[2])) < 1e-12
+    return ux, exact
+
+
+def test_p3_poiseuille_within_1pct(orc):
+    """north_star pin: laminar force-driven Poiseuille with halfway bounce-back within 1 %."""
+    ux, exact = _poiseuille(orc, 0.05, "bounce_back")
+    assert np.max(np.abs(ux - exact)) / exact.max() < 0.002
+    # the residual is the known uniform bounce-back slip (a constant offset of about -2.3e-6); it is
+    # 1.4 % of the tiny velocity of the wall-adjacent row and < 1 % pointwise everywhere else
+    assert np.max(np.abs(ux - exact)[1:-1] / exact[1:-1]) < 0.01
+
+
+def test_p3_poiseuille_magic_lambda_exact(orc):
+    """For BGK with (tau - 1/2)^2 = 3/16 the halfway bounce-back wall sits exactly half a cell
+    outside the first row for a parabolic profile: the discrete solution IS the parabola.
+    Pins tau0 = 3 nu + 1/2 (R3), the Guo prefactor and the wall location (R11) sharply."""
+    nu = np.sqrt(3.0 / 16.0) / 3.0
+    ux, exact = _poiseuille(orc, nu, "bounce_back", efolds=24.0)
+    assert np.max(np.abs(ux - exact) / exact) < 1e-9
+
+
+def test_p3_half_channel_free_slip(orc):
+    nu = np.sqrt(3.0 / 16.0) / 3.0
+    ux, exact = _poiseuille(orc, nu, "free_slip", ny=16, efolds=24.0)
+    assert np.max(np.abs(ux - exact) / exact) < 1e-9
+
+
+def test_p4_taylor_green_decay(orc):
+    """north_star pin: KE(t)/KE(0) within 1 % of exp(-2 nu |k|^2 t), |k|^2 = kx^2 + ky^2."""
+    N, nu, U0 = 48, 0.02, 0.01
+    k = 2 * np.pi / N
+    o = orc.Oracle(N, N, 2, nu, 0.0, (0, 0, 0), 0.0, None, _periodic_bc(orc))
+    X = np.arange(N)[None, None, :] + 0.0
+    Y = np.arange(N)[None, :, None] + 0.0
+    u = np.zeros((3, 2, N, N))
+    u[0] = U0 * np.sin(k * X) * np.cos(k * Y)
+    u[1] = -U0 * np.cos(k * X) * np.sin(k * Y)
+    rho = 1 + 0.75 * U0 ** 2 * (np.cos(2 * k * X) + np.cos(2 * k * Y)) + np.zeros((2, N, N))
+    o.set_macros(rho, u)
+    ke0 = None
+    t_end = int(1.0 / (2 * nu * 2 * k * k))
+    t = 0
+    for t_next in np.linspace(0, t_end, 6).astype(int):
+        o.step(int(t_next - t))
+        t = int(t_next)
+        r, v = o.get_macros()
+        ke = 0.5 * np.sum(r * (v ** 2).sum(0))
+        if ke0 is None:
+            ke0 = ke
+            continue
+        assert ke / ke0 == pytest.approx(np.exp(-2 * nu * 2 * k * k * t), rel=0.01)
+    assert ke / ke0 < 0.4   # it really decayed (wrong collision sign, R1, diverges instead)
+
+
+# ------------------------------------------------------------------------------------------
+# P5 momentum increment, P6 drag recurrence
+# ------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("Cs", [0.0, 0.17])
+def test_p5_momentum_increment_is_exactly_F(orc, Cs):
+    """One uniformly forced step adds exactly N*F to sum_cells sum_i f_i c_i (north_star), also
+    with Cs > 0 on a sheared, non-equilibrium state (pins R10: tau_total in Eq. 4 too)."""
+    c, w, _, _ = orc.tables()
+    nx, ny, nz = 6, 5, 4
+    F = np.array([3e-5, -1e-5, 2e-5])
+    o = orc.Oracle(nx, ny, nz, 2e-3, Cs, F, 0.0, None, _periodic_bc(orc))
+    rng = np.random.default_rng(5)
+    f = w[:, None, None, None] * (1 + 0.2 * rng.uniform(-1, 1, (19, nz, ny, nx)))
+    o.set_populations(f)
+    mom = lambda g: np.einsum("izyx,ia->a", g, c)
+    m0 = mom(f)
+    for step in range(1, 4):
+        o.step(1)
+        m = mom(o.get_populations())
+        assert np.allclose(m - m0, step * nx * ny * nz * F, rtol=0, atol=1e-13)
+    assert abs(o.get_populations().sum() - f.sum()) < 1e-11
+
+
+@pytest.mark.parametrize("vector", [False, True])
+def test_p6_uniform_flow_drag_recurrence(orc, vector):
+    """Alg. 1 ordering (R6, R7) and Eq. 13 (R4, R5): on a uniform periodic state streaming is
+    the identity, so the bare momentum obeys m_{n+1} = m_n + F_b + F_f(u*_n) exactly."""
+    Cd, a, rho0 = 0.2, 0.3, 1.03
+    Fb = np.array([2e-5, 0.0, -1e-5])
+    u0 = np.array([0.06, 0.02, -0.03])
+    ny = 4
+    o = orc.Oracle(4, ny, 4, 1e-3, 0.1, Fb, Cd, np.full(ny, a), _periodic_bc(orc, vector))
+    o.set_macros(np.full((4, ny, 4), rho0), u0[:, None, None, None] * np.ones((3, 4, ny, 4)))
+    m = rho0 * u0
+    for n in range(60):
+        ustar = (m + 0.5 * Fb) / rho0
+        mag = np.sqrt(ustar @ ustar)
+        Ff = -Cd * a * mag * (ustar if vector else np.array([ustar[0], 0, 0]))
+        un = ustar + 0.5 * Ff / rho0
+        rho, u = o.get_macros()
+        assert np.max(np.abs(rho - rho0)) < 1e-14
+        assert np.max(np.abs(u - un[:, None, None, None])) < 1e-15
+        o.step(1)
+        m = m + Fb + Ff
+    # continuum limit with Fb = 0, u || x: u(t) ~ u0 / (1 + Cd a u0 t)
+    o2 = orc.Oracle(4, ny, 4, 1e-3, 0.1, (0, 0, 0), Cd, np.full(ny, a), _periodic_bc(orc, vector))
+    o2.set_macros(np.ones((4, ny, 4)), np.array([0.05, 0, 0])[:, None, None, None] * np.ones((3, 4, ny, 4)))
+    o2.step(400)
+    u400 = o2.get_macros()[1][0].mean()
+    assert u400 == pytest.approx(0.05 / (1 + Cd * a * 0.05 * 400), rel=5e-3)
+
+
+# ------------------------------------------------------------------------------------------
+# P8 mirror equivalence (free-slip == symmetry plane)
+# ------------------------------------------------------------------------------------------
+
+def test_p8_free_slip_equals_mirrored_full_channel(orc):
+    cfg = wl.small(12, 8, 6, nu=5e-4, Fx=4e-6, forest_rows=2)
+    ny = cfg["ny"]
+    half = orc.Oracle.from_config(cfg)
+    lad_h = orc.lad_from_spec(cfg["forest"], ny)
+    lad_f = np.concatenate([lad_h, lad_h[::-1]])
+    full = orc.Oracle(cfg["nx"], 2 * ny, cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                      lad_f, orc.bc_flags("bounce_back", "bounce_back"))
+    i = cfg["init"]
+    rho, u = half.init_field(i["kind"], i["U_ref"], i["noise_frac"], cfg["seed"])
+    rho = rho + 0.01 * u[2]          # non-trivial density too
+    half.set_macros(rho, u)
+    um = u[:, :, ::-1, :].copy()
+    um[1] *= -1
+    full.set_macros(np.concatenate([rho, rho[:, ::-1, :]], axis=1), np.concatenate([u, um], axis=2))
+    for _ in range(4):
+        half.step(50)
+        full.step(50)
+        rh, uh = half.get_macros()
+        rf, uf = full.get_macros()
+        assert np.max(np.abs(rf[:, :ny] - rh)) < 1e-13
+        assert np.max(np.abs(uf[:, :, :ny] - uh)) < 1e-13
+        # and the full channel stayed mirror symmetric
+        assert np.max(np.abs(uf[0][:, ny:] - uf[0][:, :ny][:, ::-1])) < 1e-13
+        assert np.max(np.abs(uf[1][:, ny:] + uf[1][:, :ny][:, ::-1])) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# P9 statistics
+# ------------------------------------------------------------------------------------------
+
+def test_p9_stats_match_numpy_on_sampled_fields(orc):
+    """O10: plane sums of the sample S_k and the <ab> - <a><b> read-out, re-computed with numpy
+    reductions from the fields get_macros returns before each sampled step."""
+    cfg = wl.small(16, 10, 8, nu=5e-4, Fx=4e-6)
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    o.step(5)
+    o.stats_accumulate(2)            # sample every 2nd step, starting with the next one
+    samples = []
+    for k in range(7):
+        if k % 2 == 0:
+            samples.append(o.get_macros())
+        o.step(1)
+    out, n = o.stats_read()
+    assert n == 4 == len(samples)
+    U = np.stack([s[1] for s in samples])          # (n, 3, nz, ny, nx)
+    R = np.stack([s[0] for s in samples])
+    mean = U.mean(axis=(0, 2, 4))                  # (3, ny)
+    assert np.allclose(out[:, 0:3], mean.T, rtol=0, atol=1e-15)
+    for col, (a, b) in zip(range(3, 9), [(0, 0), (1, 1), (2, 2), (0, 1), (1, 2), (0, 2)]):
+        cov = (U[:, a] * U[:, b]).mean(axis=(0, 1, 3)) - mean[a] * mean[b]
+        assert np.allclose(out[:, col], cov, rtol=0, atol=1e-15)
+    assert np.allclose(out[:, 9], R.mean(axis=(0, 1, 3)), rtol=0, atol=1e-14)
+    o.stats_reset()
+    assert o.stats_read()[1] == 0
+
+
+def test_p9_stats_uniform_state_closed_form(orc):
+    """Uniform periodic state: plane mean = the uniform sample velocity, all stresses = 0."""
+    ny = 3
+    u0 = np.array([0.04, -0.01, 0.02])
+    o = orc.Oracle(4, ny, 4, 1e-3, 0.1, (0, 0, 0), 0.0, None, _periodic_bc(orc))
+    o.set_macros(np.full((4, ny, 4), 1.01), u0[:, None, None, None] * np.ones((3, 4, ny, 4)))
+    o.stats_accumulate(1)
+    o.step(6)
+    out, n = o.stats_read()
+    assert n == 6
+    assert np.allclose(out[:, 0:3], u0[None, :], atol=1e-16)
+    assert np.max(np.abs(out[:, 3:9])) < 1e-17
+    assert np.allclose(out[:, 9], 1.01, atol=1e-15)
+
+
+# ------------------------------------------------------------------------------------------
+# P12 symmetries, P13 brute-force push streaming
+# ------------------------------------------------------------------------------------------
+
+def test_p12_z_mirror_and_translation(orc):
+    cfg = wl.small(12, 8, 10, nu=5e-4, Fx=4e-6)
+    i = cfg["init"]
+    a = orc.Oracle.from_config(cfg)
+    rho, u = a.init_field(i["kind"], i["U_ref"], i["noise_frac"], cfg["seed"])
+    # translation in x and z of the initial field translates the result
+    b = orc.Oracle.from_config(cfg)
+    a.set_macros(rho, u)
+    b.set_macros(np.roll(rho, (3, 5), axis=(0, 2)), np.roll(u, (3, 5), axis=(1, 3)))
+    a.step(60)
+    b.step(60)
+    ra, ua = a.get_macros()
+    rb, ub = b.get_macros()
+    assert np.max(np.abs(np.roll(ra, (3, 5), axis=(0, 2)) - rb)) < 1e-14
+    assert np.max(np.abs(np.roll(ua, (3, 5), axis=(1, 3)) - ub)) < 1e-14
+    # z-mirror-symmetric initial field stays z-mirror symmetric
+    us = 0.5 * (u + u[:, ::-1] * np.array([1, 1, -1])[:, None, None, None])
+    c = orc.Oracle.from_config(cfg)
+    c.set_macros(0.5 * (rho + rho[::-1]), us)
+    c.step(60)
+    rc, uc = c.get_macros()
+    assert np.max(np.abs(rc - rc[::-1])) < 1e-14
+    assert np.max(np.abs(uc[0] - uc[0][::-1])) < 1e-14
+    assert np.max(np.abs(uc[2] + uc[2][::-1])) < 1e-14
+    assert np.abs(uc[2]).max() > 1e-6
+
+
+def _push_stream(f, c, opp, mir, bottom, top):
+    """Independent PUSH formulation: every post-collision population leaves its source cell and
+    lands at source + c_i; a wall face sends it back into the source cell reversed; a free-slip
+    face reflects its y-velocity and lets it land at the tangentially displaced cell."""
+    Q, nz, ny, nx = f.shape
+    out = np.full_like(f, np.nan)
+    for z in range(nz):
+        for y in range(ny):
+            for x in range(nx):
+                for i in range(Q):
+                    xd, yd, zd = (x + c[i, 0]) % nx, y + c[i, 1], (z + c[i, 2]) % nz
+                    j = i
+                    if yd < 0:
+                        if bottom == "periodic":
+                            yd = ny - 1
+                        else:
+                            xd, yd, zd, j = x, y, z, opp[i]
+                    elif yd >= ny:
+                        if top == "periodic":
+                            yd = 0
+                        elif top == "free_slip":
+                            yd, j = y, mir[i]
+                        else:
+                            xd, yd, zd, j = x, y, z, opp[i]
+                    assert np.isnan(out[j, zd, yd, xd])      # every slot is filled exactly once
+                    out[j, zd, yd, xd] = f[i, z, y, x]
+    assert not np.isnan(out).any()
+    return out
+
+
+@pytest.mark.parametrize("bottom,top", [("bounce_back", "bounce_back"), ("bounce_back", "free_slip"),
+                                        ("periodic", "periodic")])
+@pytest.mark.parametrize("shape", [(4, 4, 4), (5, 3, 2), (3, 1, 3)])
+def test_p13_stream_against_brute_force_push(orc, bottom, top, shape):
+    nx, ny, nz = shape
+    c, w, opp, mir = orc.tables()
+    o = orc.Oracle(nx, ny, nz, 1e-3, 0.1, (0, 0, 0), 0.0, None, orc.bc_flags(bottom, top))
+    f = np.random.default_rng(13).uniform(0.01, 1.0, (19, nz, ny, nx))
+    o.set_populations(f)
+    got = o.stream_only()
+    assert np.array_equal(got, _push_stream(f, c, opp, mir, bottom, top))
+
+
+def test_create_rejects_bad_arguments(orc):
+    with pytest.raises(ValueError):
+        orc.Oracle(4, 4, 4, -1.0, 0.1)
+    with pytest.raises(ValueError):
+        orc.Oracle(4, 4, 4, 1e-3, 0.1, bc=orc.BOTTOM_PERIODIC | orc.TOP_WALL)
