@@ -1,0 +1,168 @@
+/* lbm.h — C ABI of the B200-native fused D3Q19 LES + forest-canopy lattice Boltzmann step.
+ *
+ * Method: arxiv 2206.15454 (Shao et al.), Algorithm 1 with Eqs. 1-16:
+ *   stream (Eq. 1) -> moments (Eqs. 5-7) -> forest drag F_f = -C_D a_f(y)|u|u
+ *   (Eq. 13) with the half-force velocity shift (Eq. 6) -> Smagorinsky relaxation
+ *   time from the local non-equilibrium momentum flux (Eqs. 10-12) -> BGK collision
+ *   (Eqs. 2-3) with Guo forcing (Eq. 4); periodic x/z and no-slip wall without a
+ *   wall function (L177, L216); time + x-z-plane averages of velocity and stresses (L200, L251).
+ *   The readings of ambiguous passages are listed in DESIGN.md ("Readings", R1..R26).
+ *
+ * Conventions
+ *   - Lattice units: dx = dt = 1, c_s^2 = 1/3.  x streamwise, y wall-normal, z spanwise.
+ *   - cell = x + nx*(y + ny*z) (x fastest).  All ny rows are fluid; the bottom boundary plane is
+ *     the face below row 0 and the top boundary plane the face above row ny-1 (halfway links).
+ *   - x and z are always periodic.
+ *   - Every call returns LBM_OK (0) or a negative lbm_status; no exception or abort crosses the
+ *     ABI.  lbm_last_error() returns a thread-local, NUL-terminated description of the last
+ *     failure on the calling thread.
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host pointers.  The
+ *     library never allocates population memory: the caller (the Python binding uses
+ *     torch.empty) owns one device workspace of lbm_workspace_bytes() bytes, 256-byte aligned,
+ *     and must keep it alive until lbm_destroy.  All kernels are launched on the CUDA stream
+ *     given to lbm_bind (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *   - All calls on one handle must come from one host thread at a time.
+ *   - Time: "state k" is the post-collision population set after k steps.  The sample
+ *     S_k = (rho, u) is obtained by streaming state k and applying Eqs. 5-6 and 13 (what step
+ *     k+1 sees before colliding; reading R19).  lbm_step(1) maps state k -> k+1 and, when
+ *     statistics are on and due, accumulates S_k.  lbm_get_macros returns S_k, state unchanged.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbm_s lbm_t; /* opaque, owned by the library */
+
+typedef enum lbm_status {
+    LBM_OK = 0,
+    LBM_EINVAL = -1,    /* bad argument (size, nu <= 0, NULL pointer, unsupported flag combination) */
+    LBM_ENOMEM = -2,    /* workspace too small / misaligned, or host allocation failed */
+    LBM_ESTATE = -3,    /* call out of order (step before bind/init, ...) */
+    LBM_ECUDA = -4,     /* CUDA runtime error; text in lbm_last_error() */
+    LBM_EDIVERGED = -5  /* a non-finite density was seen by the statistics / macros reduction */
+} lbm_status;
+
+/* bc_flags bit field */
+#define LBM_BOTTOM_WALL       0u          /* bits 0-1: halfway bounce-back no-slip wall (L177, L216) */
+#define LBM_BOTTOM_PERIODIC   1u          /*           periodic in y (closed-form test cases only)   */
+#define LBM_TOP_WALL          (0u << 2)   /* bits 2-3: halfway bounce-back                            */
+#define LBM_TOP_FREE_SLIP     (1u << 2)   /*           specular reflection (BASELINE.json configs)    */
+#define LBM_TOP_PERIODIC      (2u << 2)   /*           periodic in y (must pair with BOTTOM_PERIODIC) */
+#define LBM_DRAG_VECTOR       (1u << 4)   /* bit 4: 0 streamwise-only drag (paper, L98/L103), 1 vector */
+#define LBM_STORAGE_AA        (1u << 6)   /* bit 6: 0 two-lattice pull, 1 single-array AA pattern     */
+#define LBM_VEC_SHIFT         8           /* bits 8-10: cells per thread override (0 auto, 1, 2, 4)   */
+#define LBM_VEC_MASK          (7u << 8)
+
+#define LBM_NSTAT 10 /* columns of lbm_stats_read */
+
+/* Initial-profile kinds for lbm_set_init */
+#define LBM_INIT_POWER_LAW 0 /* U_ref * ((j+1/2)/ny)^(1/7) e_x */
+#define LBM_INIT_PARABOLA  1 /* U_ref * 4 eta (1-eta) e_x, eta = (j+1/2)/ny */
+#define LBM_INIT_REST      2 /* u = 0 */
+
+/* Bytes of device workspace a handle with these sizes/flags needs (populations: 76 B/cell for
+ * AA, 152 B/cell for two-lattice; plus statistics partials, tables and a host-transfer staging
+ * area).  Host call, no CUDA work. */
+int lbm_workspace_bytes(int nx, int ny, int nz, uint32_t bc_flags, size_t *bytes);
+
+/* Create a handle.  Problem statement of Alg. 1's inputs (L140) and Table I/II parameters:
+ *   nu          kinematic viscosity, lattice units, > 0; tau0 = 3 nu + 1/2 (R3)
+ *   Cs          Smagorinsky constant; the paper's C_smag (Eq. 9) equals Cs^2 (R9)
+ *   body_force  host, 3 doubles, force DENSITY F_b (Eq. 16; R4); copied; NULL = 0
+ *   Cd          drag coefficient C_D of Eq. 13
+ *   lad_profile host, ny doubles a_f(y_j) at cell centres y_j = j + 1/2 (Eqs. 14-15 evaluated by
+ *               the caller, or lbm_lad_profile below); copied; NULL or all-zero = no forest
+ * Host call; needs a CUDA device only at lbm_bind.  Errors: LBM_EINVAL, LBM_ENOMEM. */
+int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs,
+               const double *body_force, double Cd, const double *lad_profile,
+               uint32_t bc_flags);
+
+/* Attach the caller-owned device workspace and stream; uploads the per-row tables.
+ * Errors: LBM_ENOMEM (bytes < lbm_workspace_bytes or pointer not 256-B aligned), LBM_ECUDA. */
+int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream);
+
+/* Choose the synthetic initial field used by lbm_init (R16): rho = 1,
+ * u = U(y_j) e_x + noise_frac*U_ref*(2r-1) per component, r = rand01(seed, 3*cell+comp). */
+int lbm_set_init(lbm_t *h, int kind, double U_ref, double noise_frac);
+
+/* State 0: f = f_eq(1, u_init) (Eq. 3; R17); t = 0; statistics cleared.  Async on the stream. */
+int lbm_init(lbm_t *h, uint64_t seed);
+
+/* State 0 from caller fields: f = f_eq(rho, u).  rho: [nz][ny][nx] fp32, u: [3][nz][ny][nx] fp32.
+ * _dev: device pointers (read asynchronously on the stream).  _host: host pointers, copied
+ * through the workspace staging area (pinned memory makes the copies asynchronous); returns
+ * after the last copy has been consumed. */
+int lbm_set_macros(lbm_t *h, const float *rho_dev, const float *u_dev);
+int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host);
+
+/* Advance n >= 0 time steps: one fused kernel launch per step (stream, moments, drag,
+ * Smagorinsky tau, Guo-forced BGK collision, boundary links, store; plus the fused stage-1
+ * plane sums and the stage-2 reduction kernel on sampled steps).  Asynchronous. */
+int lbm_step(lbm_t *h, int n);
+
+/* Sample S_k of the current state (see "Time" above) into caller-owned buffers (layouts as in
+ * lbm_set_macros).  Either pointer may be NULL.  _dev is asynchronous; _host synchronises. */
+int lbm_get_macros(lbm_t *h, float *rho_dev, float *u_dev);
+int lbm_get_macros_host(lbm_t *h, float *rho_host, float *u_host);
+
+/* Statistics (L200, L251: time then x-z plane averaging; L210 needs <v'w'>).
+ * lbm_stats_accumulate(every): every > 0 samples S_k on every every-th step taken by lbm_step
+ * from now on (phase restarts), every == 0 switches sampling off.  Sums are kept.
+ * lbm_stats_read: synchronises the stream; out is host [ny][LBM_NSTAT] doubles, columns
+ *   <u>, <v>, <w>, <u'u'>, <v'v'>, <w'w'>, <u'v'>, <v'w'>, <u'w'>, <rho>,
+ * with <a> = sum a / (nsamples nx nz) and <a'b'> = <ab> - <a><b> (R18); *nsamples may be NULL.
+ * Returns LBM_EDIVERGED if a non-finite plane sum was seen.
+ * lbm_stats_reset clears the sums and re-centres the accumulation about the current plane
+ * means (a numerical shift only; results are unchanged up to rounding). */
+int lbm_stats_accumulate(lbm_t *h, int every);
+int lbm_stats_read(lbm_t *h, double *out_host, long long *nsamples);
+int lbm_stats_reset(lbm_t *h);
+
+/* Raw copy of the population array(s) in the library's internal representation, for
+ * checkpointing and tests: device [19][nz][ny][nx] fp32 of f_i - w_i in SPECIFICATION numbering
+ * (include/lbm.h velocity table below), converted to the plain "state k" (post-collision,
+ * un-streamed) representation whatever the storage mode/parity. */
+int lbm_get_state(lbm_t *h, float *f_minus_w_dev);
+
+/* Number of steps taken since the last init / set_macros. */
+long long lbm_time(const lbm_t *h);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+long long lbm_launch_count(const lbm_t *h);
+
+/* Tuning hook: override the thread-block shape (tx thread columns of V cells along x, ty rows;
+ * tx*ty <= 256, tx divides nx/V with at most 8 blocks per row, ty divides ny*nz).  Call before
+ * the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
+int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
+
+/* Name of the kernel variant lbm_step uses, e.g. "aa/v4/tx384x1" (static string per handle). */
+const char *lbm_variant(const lbm_t *h);
+
+void lbm_destroy(lbm_t *h);
+
+const char *lbm_last_error(void);
+
+/* Host helpers (no CUDA): leaf-area-density table of Eqs. 14-15 (L105-115; R14):
+ * a_j = LAI * s(eta_j) / sum_k s(eta_k) for j < h, 0 above, eta_j = (j+1/2)/h,
+ * s(eta) = r^n exp[n(1-r)], r = (1-eta_m)/(1-eta), n = 6 (eta < eta_m) or 1/2. */
+int lbm_lad_profile(int h, int ny, double LAI, double eta_m, double *out_host);
+
+/* Counter-based uniform generator of the input recipe: splitmix64 output function of
+ * seed + (ctr+1)*0x9E3779B97F4A7C15; rand01 = top 53 bits * 2^-53. */
+uint64_t lbm_mix64(uint64_t seed, uint64_t ctr);
+
+/* D3Q19 numbering used by every external layout:
+ *  0:(0,0,0) | 1:(+,0,0) 2:(-,0,0) 3:(0,+,0) 4:(0,-,0) 5:(0,0,+) 6:(0,0,-) |
+ *  7:(+,+,0) 8:(-,-,0) 9:(+,-,0) 10:(-,+,0) 11:(+,0,+) 12:(-,0,-) 13:(+,0,-) 14:(-,0,+)
+ *  15:(0,+,+) 16:(0,-,-) 17:(0,+,-) 18:(0,-,+);  w = 1/3, 1/18 (1-6), 1/36 (7-18). */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

@@ -1,0 +1,284 @@
+"""Thin ctypes binding of the C ABI in include/lbm.h (argument marshalling only).
+
+PyTorch is used for exactly two things: the device workspace (`torch.empty(..., device="cuda")`)
+and the CUDA stream the kernels are launched on.  Every step of the method runs in the CUDA
+library; there is no CPU fallback: if the shared object or a GPU is missing the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+# bc_flags (mirrors include/lbm.h)
+BOTTOM_WALL, BOTTOM_PERIODIC = 0, 1
+TOP_WALL, TOP_FREE_SLIP, TOP_PERIODIC = 0 << 2, 1 << 2, 2 << 2
+DRAG_VECTOR = 1 << 4
+STORAGE_AA = 1 << 6
+VEC_SHIFT = 8
+NSTAT = 10
+
+INIT_POWER_LAW, INIT_PARABOLA, INIT_REST = 0, 1, 2
+
+LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ESTATE, LBM_ECUDA, LBM_EDIVERGED = 0, -1, -2, -3, -4, -5
+
+_BOTTOM = {"bounce_back": BOTTOM_WALL, "periodic": BOTTOM_PERIODIC}
+_TOP = {"bounce_back": TOP_WALL, "free_slip": TOP_FREE_SLIP, "periodic": TOP_PERIODIC}
+
+# every symbol include/lbm.h declares
+SYMBOLS = [
+    "lbm_workspace_bytes", "lbm_create", "lbm_bind", "lbm_set_init", "lbm_init", "lbm_set_macros",
+    "lbm_set_macros_host", "lbm_step", "lbm_get_macros", "lbm_get_macros_host",
+    "lbm_stats_accumulate", "lbm_stats_read", "lbm_stats_reset", "lbm_get_state", "lbm_time",
+    "lbm_launch_count", "lbm_set_launch_shape", "lbm_variant", "lbm_destroy", "lbm_last_error",
+    "lbm_lad_profile", "lbm_mix64",
+]
+
+
+class LbmError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"lbm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load (building if needed) liblbm_b200.so.  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB if (os.path.exists(_build.LIB) and not _build.needs_build()) else _build.build()
+        L = C.CDLL(path)
+        vp, dp, fp = C.c_void_p, C.POINTER(C.c_double), C.c_void_p
+        L.lbm_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_uint32, C.POINTER(C.c_size_t)]
+        L.lbm_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, dp,
+                                 C.c_double, dp, C.c_uint32]
+        L.lbm_bind.argtypes = [vp, vp, C.c_size_t, vp]
+        L.lbm_set_init.argtypes = [vp, C.c_int, C.c_double, C.c_double]
+        L.lbm_init.argtypes = [vp, C.c_uint64]
+        L.lbm_set_macros.argtypes = [vp, fp, fp]
+        L.lbm_set_macros_host.argtypes = [vp, fp, fp]
+        L.lbm_step.argtypes = [vp, C.c_int]
+        L.lbm_get_macros.argtypes = [vp, fp, fp]
+        L.lbm_get_macros_host.argtypes = [vp, fp, fp]
+        L.lbm_stats_accumulate.argtypes = [vp, C.c_int]
+        L.lbm_stats_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.lbm_stats_reset.argtypes = [vp]
+        L.lbm_get_state.argtypes = [vp, fp]
+        L.lbm_time.argtypes = [vp]
+        L.lbm_time.restype = C.c_longlong
+        L.lbm_launch_count.argtypes = [vp]
+        L.lbm_launch_count.restype = C.c_longlong
+        L.lbm_set_launch_shape.argtypes = [vp, C.c_int, C.c_int]
+        L.lbm_variant.argtypes = [vp]
+        L.lbm_variant.restype = C.c_char_p
+        L.lbm_destroy.argtypes = [vp]
+        L.lbm_destroy.restype = None
+        L.lbm_last_error.restype = C.c_char_p
+        L.lbm_lad_profile.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
+        L.lbm_mix64.argtypes = [C.c_uint64, C.c_uint64]
+        L.lbm_mix64.restype = C.c_uint64
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise LbmError(rc, lib().lbm_last_error().decode())
+
+
+def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa: bool = False, vec: int = 0) -> int:
+    return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0) | (STORAGE_AA if aa else 0)
+            | (int(vec) << VEC_SHIFT))
+
+
+def workspace_bytes(nx: int, ny: int, nz: int, flags: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().lbm_workspace_bytes(nx, ny, nz, flags, C.byref(out)))
+    return int(out.value)
+
+
+def lad_profile(h: int, ny: int, LAI: float, eta_m: float = 0.7) -> np.ndarray:
+    out = np.zeros(ny)
+    _check(lib().lbm_lad_profile(int(h), int(ny), float(LAI), float(eta_m),
+                                 out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
+def mix64(seed: int, ctr: int) -> int:
+    return int(lib().lbm_mix64(C.c_uint64(seed), C.c_uint64(ctr)))
+
+
+def lad_from_spec(forest, ny: int):
+    """lad_profile table from a workloads forest spec (None / uniform / lalic)."""
+    if forest is None:
+        return None
+    if forest["kind"] == "uniform":
+        a = np.zeros(ny)
+        a[: forest["rows"]] = forest["a"]
+        return a
+    if forest["kind"] == "lalic":
+        return lad_profile(forest["h"], ny, forest["LAI"], forest.get("eta_m", 0.7))
+    raise ValueError(forest)
+
+
+class Lbm:
+    """One simulation handle.  Arrays: rho (nz, ny, nx), u (3, nz, ny, nx), float32."""
+
+    def __init__(self, nx, ny, nz, nu, Cs, body_force=(0.0, 0.0, 0.0), Cd=0.0, lad=None, flags=0,
+                 device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2206_15454_b200 needs a CUDA device; there is no CPU fallback")
+        L = lib()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.N = self.nx * self.ny * self.nz
+        self.flags = int(flags)
+        self.device = torch.device(device)
+        bf = np.ascontiguousarray(body_force, dtype=np.float64)
+        dp = C.POINTER(C.c_double)
+        ladp = None
+        if lad is not None:
+            lad = np.ascontiguousarray(lad, dtype=np.float64)
+            if lad.shape != (self.ny,):
+                raise ValueError("lad must have ny entries")
+            ladp = lad.ctypes.data_as(dp)
+        h = C.c_void_p()
+        _check(L.lbm_create(C.byref(h), self.nx, self.ny, self.nz, float(nu), float(Cs),
+                            bf.ctypes.data_as(dp), float(Cd), ladp, self.flags))
+        self._h = h
+        nbytes = workspace_bytes(self.nx, self.ny, self.nz, self.flags)
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        base = self._ws.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        _check(L.lbm_bind(self._h, C.c_void_p(aligned), C.c_size_t(nbytes), C.c_void_p(self._stream.cuda_stream)))
+
+    @classmethod
+    def from_config(cls, cfg: dict, aa=None, vec: int = 0, **kw) -> "Lbm":
+        if aa is None:
+            aa = cfg.get("storage", "two_lattice") == "aa"
+        flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec)
+        s = cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                lad_from_spec(cfg["forest"], cfg["ny"]), flags, **kw)
+        i = cfg["init"]
+        s.set_init(i["kind"], i["U_ref"], i["noise_frac"])
+        return s
+
+    def close(self):
+        h = getattr(self, "_h", None)
+        if h:
+            lib().lbm_destroy(h)
+            self._h = None
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def shape(self):
+        return (self.nz, self.ny, self.nx)
+
+    @property
+    def variant(self) -> str:
+        return lib().lbm_variant(self._h).decode()
+
+    @property
+    def time(self) -> int:
+        return int(lib().lbm_time(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().lbm_launch_count(self._h))
+
+    def set_launch_shape(self, tx: int, ty: int):
+        _check(lib().lbm_set_launch_shape(self._h, int(tx), int(ty)))
+
+    def set_init(self, kind: int, U_ref: float, noise_frac: float):
+        _check(lib().lbm_set_init(self._h, int(kind), float(U_ref), float(noise_frac)))
+
+    def init(self, seed: int):
+        _check(lib().lbm_init(self._h, C.c_uint64(seed)))
+
+    def _dev(self, t, shape):
+        import torch
+
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                and tuple(t.shape) == tuple(shape)):
+            raise ValueError(f"expected a contiguous float32 CUDA tensor of shape {shape}")
+        return C.c_void_p(t.data_ptr())
+
+    @staticmethod
+    def _host(a, shape):
+        import torch
+
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+                raise ValueError(f"expected a contiguous float32 CPU tensor of shape {shape}")
+            return C.c_void_p(a.data_ptr())
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags["C_CONTIGUOUS"]
+                and a.shape == tuple(shape)):
+            raise ValueError(f"expected a C-contiguous float32 array of shape {shape}")
+        return C.c_void_p(a.ctypes.data)
+
+    def set_macros(self, rho, u):
+        """State 0 = f_eq(rho, u) from CUDA tensors."""
+        _check(lib().lbm_set_macros(self._h, self._dev(rho, self.shape), self._dev(u, (3,) + self.shape)))
+
+    def set_macros_host(self, rho, u):
+        """State 0 = f_eq(rho, u) from host arrays (numpy or CPU tensors; pinned = async copies)."""
+        _check(lib().lbm_set_macros_host(self._h, self._host(rho, self.shape), self._host(u, (3,) + self.shape)))
+
+    def step(self, n: int = 1):
+        _check(lib().lbm_step(self._h, int(n)))
+
+    def get_macros(self, rho=None, u=None):
+        """Sample S_k into CUDA tensors (allocated with torch if not given)."""
+        import torch
+
+        if rho is None:
+            rho = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        if u is None:
+            u = torch.empty((3,) + self.shape, dtype=torch.float32, device=self.device)
+        _check(lib().lbm_get_macros(self._h, self._dev(rho, self.shape), self._dev(u, (3,) + self.shape)))
+        return rho, u
+
+    def get_macros_host(self, rho=None, u=None):
+        if rho is None:
+            rho = np.empty(self.shape, dtype=np.float32)
+        if u is None:
+            u = np.empty((3,) + self.shape, dtype=np.float32)
+        _check(lib().lbm_get_macros_host(self._h, self._host(rho, self.shape), self._host(u, (3,) + self.shape)))
+        return rho, u
+
+    def get_state(self):
+        """(19, nz, ny, nx) CUDA tensor of f_i - w_i, plain post-collision state."""
+        import torch
+
+        out = torch.empty((19,) + self.shape, dtype=torch.float32, device=self.device)
+        _check(lib().lbm_get_state(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def stats_accumulate(self, every: int = 1):
+        _check(lib().lbm_stats_accumulate(self._h, int(every)))
+
+    def stats_reset(self):
+        _check(lib().lbm_stats_reset(self._h))
+
+    def stats_read(self):
+        out = np.zeros((self.ny, NSTAT))
+        n = C.c_longlong(0)
+        _check(lib().lbm_stats_read(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
+        return out, int(n.value)
+
+    def synchronize(self):
+        self._stream.synchronize()

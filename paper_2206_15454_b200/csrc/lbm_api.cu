@@ -1,0 +1,562 @@
+// lbm_api.cu — host side of the C ABI declared in include/lbm.h: argument checking, workspace
+// layout, kernel dispatch.  No torch types; the caller owns the device workspace and the stream.
+#include "../../include/lbm.h"
+#include "lbm_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace lbm;
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU_TRY(expr)                                                                          \
+    do {                                                                                      \
+        cudaError_t e__ = (expr);                                                             \
+        if (e__ != cudaSuccess)                                                               \
+            return fail(LBM_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));          \
+    } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+constexpr int MAX_NCHUNK = 8;
+constexpr size_t STAGING_BUDGET = (size_t)256 << 20;
+
+struct Layout {
+    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, staging, total;
+    int stage_planes;
+};
+
+static Layout make_layout(int nx, int ny, int nz, bool aa)
+{
+    Layout L;
+    const size_t N = (size_t)nx * ny * nz;
+    size_t off = 0;
+    L.pops = off; off = align_up(off + (size_t)Q * N * 4, 256);
+    L.pops2 = off; if (!aa) off = align_up(off + (size_t)Q * N * 4, 256);
+    L.partial = off; off = align_up(off + (size_t)ny * NSTAT * nz * MAX_NCHUNK * 4, 256);
+    L.acc = off; off = align_up(off + (size_t)ny * NSTAT * 8, 256);
+    L.shift = off; off = align_up(off + (size_t)ny * 4 * 4, 256);
+    L.cda = off; off = align_up(off + (size_t)ny * 4, 256);
+    L.uprof = off; off = align_up(off + (size_t)ny * 4, 256);
+    L.flag = off; off += 256;
+    const size_t plane = (size_t)16 * nx * ny;
+    size_t planes = STAGING_BUDGET / plane;
+    if (planes < 1) planes = 1;
+    if (planes > (size_t)nz) planes = nz;
+    L.stage_planes = (int)planes;
+    L.staging = off; off = align_up(off + planes * plane, 256);
+    L.total = off;
+    return L;
+}
+
+struct lbm_s {
+    int nx, ny, nz;
+    long long N;
+    double nu, Cs, Fb[3], Cd;
+    std::vector<double> lad;
+    uint32_t bc;
+    int bot, top;
+    bool aa, drag_vector;
+    int V, TX, TY, nchunk;
+    Layout L;
+    char *ws;
+    cudaStream_t stream;
+    bool bound, inited;
+    long long t;
+    int stats_every;
+    long long stats_phase, nsamples;
+    long long launches;
+    int init_kind;
+    double U_ref, noise_frac;
+    char variant[64];
+    KParams kp;
+};
+
+static bool valid_top_bottom(uint32_t bc, int *bot, int *top)
+{
+    const int b = bc & 3u, t = (bc >> 2) & 3u;
+    if (b > 1 || t > 2) return false;
+    if ((b == 1) != (t == 2)) return false; // periodic-y needs both faces
+    *bot = b; *top = t;
+    return true;
+}
+
+static int pick_vec(int nx, uint32_t bc)
+{
+    const int req = (bc & LBM_VEC_MASK) >> LBM_VEC_SHIFT;
+    if (req == 1 || req == 2 || req == 4) return (nx % req == 0) ? req : -1;
+    if (req != 0) return -1;
+    if (nx % 4 == 0) return 4;
+    if (nx % 2 == 0) return 2;
+    return 1;
+}
+
+// Block shape: TX threads along x (a divisor of the nx/V thread columns of a row, at most
+// MAX_NCHUNK blocks per row, whole warps preferred), TY rows, TX*TY <= target threads.
+static bool pick_shape(int W, long long nrows, int target, int *TX, int *TY)
+{
+    int best = -1, best_score = -1;
+    for (int d = 1; d <= W && d <= target; ++d) {
+        if (W % d) continue;
+        if (W / d > MAX_NCHUNK) continue;
+        int score = d + ((d % 32 == 0) ? 100000 : 0) + ((d < 32 && (d & (d - 1)) == 0) ? 50000 : 0);
+        if (score > best_score) { best_score = score; best = d; }
+    }
+    if (best < 0) return false;
+    int ty = 1;
+    for (int d = 1; d * best <= target; ++d)
+        if (nrows % d == 0) ty = d;
+    *TX = best; *TY = ty;
+    return true;
+}
+
+// Every lbm_* function below is declared extern "C" in include/lbm.h and keeps that linkage.
+
+const char *lbm_last_error(void) { return g_err; }
+
+int lbm_workspace_bytes(int nx, int ny, int nz, uint32_t bc_flags, size_t *bytes)
+{
+    if (!bytes) return fail(LBM_EINVAL, "bytes is NULL");
+    if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "lattice sizes must be >= 1");
+    if ((double)nx * ny * nz >= 2147483648.0) return fail(LBM_EINVAL, "nx*ny*nz must be < 2^31");
+    *bytes = make_layout(nx, ny, nz, (bc_flags & LBM_STORAGE_AA) != 0).total;
+    return LBM_OK;
+}
+
+int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const double *body_force,
+               double Cd, const double *lad_profile, uint32_t bc_flags)
+{
+    if (!out) return fail(LBM_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "lattice sizes must be >= 1 (got %d %d %d)", nx, ny, nz);
+    if ((double)nx * ny * nz >= 2147483648.0) return fail(LBM_EINVAL, "nx*ny*nz must be < 2^31");
+    if (!(nu > 0.0) || !std::isfinite(nu)) return fail(LBM_EINVAL, "nu must be > 0 (got %g)", nu);
+    if (!(Cs >= 0.0) || !std::isfinite(Cs)) return fail(LBM_EINVAL, "Cs must be >= 0 (got %g)", Cs);
+    if (!(Cd >= 0.0) || !std::isfinite(Cd)) return fail(LBM_EINVAL, "Cd must be >= 0 (got %g)", Cd);
+    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_STORAGE_AA | LBM_VEC_MASK))
+        return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
+    int bot, top;
+    if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
+    const int V = pick_vec(nx, bc_flags);
+    if (V < 0) return fail(LBM_EINVAL, "cells-per-thread override does not divide nx=%d", nx);
+    lbm_s *h = new (std::nothrow) lbm_s();
+    if (!h) return fail(LBM_ENOMEM, "host allocation failed");
+    h->nx = nx; h->ny = ny; h->nz = nz; h->N = (long long)nx * ny * nz;
+    h->nu = nu; h->Cs = Cs; h->Cd = Cd;
+    for (int a = 0; a < 3; ++a) {
+        h->Fb[a] = body_force ? body_force[a] : 0.0;
+        if (!std::isfinite(h->Fb[a])) { delete h; return fail(LBM_EINVAL, "body_force[%d] is not finite", a); }
+    }
+    h->lad.assign(ny, 0.0);
+    if (lad_profile)
+        for (int j = 0; j < ny; ++j) {
+            if (!(lad_profile[j] >= 0.0) || !std::isfinite(lad_profile[j])) { delete h; return fail(LBM_EINVAL, "lad_profile[%d] must be >= 0", j); }
+            h->lad[j] = lad_profile[j];
+        }
+    h->bc = bc_flags; h->bot = bot; h->top = top;
+    h->aa = (bc_flags & LBM_STORAGE_AA) != 0;
+    h->drag_vector = (bc_flags & LBM_DRAG_VECTOR) != 0;
+    h->V = V;
+    if (!pick_shape(nx / V, (long long)ny * nz, 128, &h->TX, &h->TY)) {
+        delete h;
+        return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
+    }
+    h->nchunk = (nx / V) / h->TX;
+    h->L = make_layout(nx, ny, nz, h->aa);
+    h->ws = nullptr; h->stream = nullptr; h->bound = false; h->inited = false;
+    h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
+    h->init_kind = LBM_INIT_REST; h->U_ref = 0.0; h->noise_frac = 0.0;
+    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", V, h->TX, h->TY);
+    *out = h;
+    return LBM_OK;
+}
+
+int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    const int W = h->nx / h->V;
+    if (tx < 1 || ty < 1 || tx * ty > MAX_THREADS || W % tx || (W / tx) > MAX_NCHUNK ||
+        ((long long)h->ny * h->nz) % ty)
+        return fail(LBM_EINVAL, "launch shape %dx%d does not tile %d thread columns x %lld rows", tx, ty, W,
+                    (long long)h->ny * h->nz);
+    h->TX = tx; h->TY = ty; h->nchunk = W / tx;
+    h->kp.nchunk = h->nchunk;
+    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", h->V, h->TX, h->TY);
+    return LBM_OK;
+}
+
+static void fill_params(lbm_s *h)
+{
+    KParams &p = h->kp;
+    memset(&p, 0, sizeof(p));
+    p.src = reinterpret_cast<float *>(h->ws + h->L.pops);
+    p.dst = h->aa ? p.src : reinterpret_cast<float *>(h->ws + h->L.pops2);
+    p.nx = h->nx; p.ny = h->ny; p.nz = h->nz; p.nchunk = h->nchunk; p.N = h->N;
+    const double tau0 = 3.0 * h->nu + 0.5;              // R3
+    p.tau0 = (float)tau0; p.tau0sq = (float)(tau0 * tau0);
+    p.ksmag = (float)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs); // R9: C_smag = Cs^2
+    p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
+    p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
+    p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
+    p.partial = nullptr; p.shift = nullptr;
+    p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
+    p.z0 = 0; p.z1 = h->nz; p.zoff = 0; p.Nio = h->N;
+}
+
+int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!dev_workspace) return fail(LBM_EINVAL, "workspace is NULL");
+    if (bytes < h->L.total) return fail(LBM_ENOMEM, "workspace too small: %zu < %zu bytes", bytes, h->L.total);
+    if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) return fail(LBM_ENOMEM, "workspace must be 256-byte aligned");
+    h->ws = static_cast<char *>(dev_workspace);
+    h->stream = static_cast<cudaStream_t>(cuda_stream);
+    fill_params(h);
+    std::vector<float> cda(h->ny);
+    for (int j = 0; j < h->ny; ++j) cda[j] = (float)(h->Cd * h->lad[j]);
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.cda, cda.data(), h->ny * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream)); // cda is a local vector
+    h->bound = true; h->inited = false;
+    return LBM_OK;
+}
+
+int lbm_set_init(lbm_t *h, int kind, double U_ref, double noise_frac)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (kind < 0 || kind > 2) return fail(LBM_EINVAL, "unknown init kind %d", kind);
+    if (!std::isfinite(U_ref) || !std::isfinite(noise_frac)) return fail(LBM_EINVAL, "U_ref / noise_frac not finite");
+    h->init_kind = kind; h->U_ref = U_ref; h->noise_frac = noise_frac;
+    return LBM_OK;
+}
+
+// ---- launch helpers --------------------------------------------------------------------------
+
+template <int V>
+static cudaError_t launch_init_v(lbm_s *h, const KParams &p, int planes)
+{
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY), h->nchunk);
+    if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
+    else init_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
+}
+static cudaError_t launch_init(lbm_s *h, const KParams &p, int planes)
+{
+    switch (h->V) {
+    case 4: return launch_init_v<4>(h, p, planes);
+    case 2: return launch_init_v<2>(h, p, planes);
+    default: return launch_init_v<1>(h, p, planes);
+    }
+}
+
+template <int V>
+static cudaError_t launch_macros_v(lbm_s *h, const KParams &p, int planes)
+{
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY), h->nchunk);
+    if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
+    else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL><<<grid, block, 0, h->stream>>>(p);
+    else macros_kernel<V, RD_PULL_OPP><<<grid, block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
+}
+static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
+{
+    switch (h->V) {
+    case 4: return launch_macros_v<4>(h, p, planes);
+    case 2: return launch_macros_v<2>(h, p, planes);
+    default: return launch_macros_v<1>(h, p, planes);
+    }
+}
+
+template <int V, bool S>
+static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
+{
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY), h->nchunk);
+    if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
+    else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S><<<grid, block, 0, h->stream>>>(p);
+    else step_kernel<V, RD_PULL_OPP, WR_PUSH, S><<<grid, block, 0, h->stream>>>(p);
+    h->launches++;
+    return cudaGetLastError();
+}
+static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
+{
+    switch (h->V) {
+    case 4: return stats ? launch_step_vs<4, true>(h, p) : launch_step_vs<4, false>(h, p);
+    case 2: return stats ? launch_step_vs<2, true>(h, p) : launch_step_vs<2, false>(h, p);
+    default: return stats ? launch_step_vs<1, true>(h, p) : launch_step_vs<1, false>(h, p);
+    }
+}
+
+static cudaError_t launch_stage2(lbm_s *h, int mode)
+{
+    dim3 grid(h->ny, NSTAT);
+    stats_stage2_kernel<<<grid, 256, 0, h->stream>>>(
+        reinterpret_cast<const float *>(h->ws + h->L.partial), (long long)h->nz * h->nchunk,
+        reinterpret_cast<double *>(h->ws + h->L.acc), reinterpret_cast<float *>(h->ws + h->L.shift), mode,
+        1.0 / ((double)h->nx * h->nz), reinterpret_cast<int *>(h->ws + h->L.flag));
+    h->launches++;
+    return cudaGetLastError();
+}
+
+static int stats_reset_impl(lbm_s *h)
+{
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
+    h->nsamples = 0; h->stats_phase = 0;
+    if (h->inited) {
+        // centre the accumulation on the current plane means (numerical shift only)
+        KParams p = h->kp;
+        p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
+        p.shift = nullptr;
+        CU_TRY(launch_macros(h, p, h->nz));
+        CU_TRY(launch_stage2(h, 1));
+    }
+    return LBM_OK;
+}
+
+static int upload_profile(lbm_s *h)
+{
+    std::vector<float> up(h->ny);
+    for (int j = 0; j < h->ny; ++j) {
+        const double eta = (j + 0.5) / h->ny;
+        double U = 0.0;
+        if (h->init_kind == LBM_INIT_POWER_LAW) U = h->U_ref * std::pow(eta, 1.0 / 7.0);
+        else if (h->init_kind == LBM_INIT_PARABOLA) U = h->U_ref * 4.0 * eta * (1.0 - eta);
+        up[j] = (float)U;
+    }
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.uprof, up.data(), h->ny * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_init(lbm_t *h, uint64_t seed)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_init before lbm_bind");
+    int rc = upload_profile(h);
+    if (rc) return rc;
+    fill_params(h);
+    KParams p = h->kp;
+    p.rho_in = nullptr; p.u_in = nullptr;
+    p.noise_amp = h->noise_frac * h->U_ref;
+    p.seed = seed;
+    p.dst = p.src; // state 0 lives in the primary array
+    CU_TRY(launch_init(h, p, h->nz));
+    h->t = 0; h->inited = true;
+    return stats_reset_impl(h);
+}
+
+int lbm_set_macros(lbm_t *h, const float *rho_dev, const float *u_dev)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_macros before lbm_bind");
+    if (!rho_dev || !u_dev) return fail(LBM_EINVAL, "rho / u is NULL");
+    fill_params(h);
+    KParams p = h->kp;
+    p.rho_in = rho_dev; p.u_in = u_dev; p.dst = p.src;
+    CU_TRY(launch_init(h, p, h->nz));
+    h->t = 0; h->inited = true;
+    return stats_reset_impl(h);
+}
+
+int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_macros_host before lbm_bind");
+    if (!rho_host || !u_host) return fail(LBM_EINVAL, "rho / u is NULL");
+    fill_params(h);
+    const size_t plane = (size_t)h->nx * h->ny;
+    float *stg = reinterpret_cast<float *>(h->ws + h->L.staging);
+    for (int z0 = 0; z0 < h->nz; z0 += h->L.stage_planes) {
+        const int zc = (h->nz - z0 < h->L.stage_planes) ? h->nz - z0 : h->L.stage_planes;
+        const size_t cnt = plane * zc;
+        CU_TRY(cudaMemcpyAsync(stg, rho_host + plane * z0, cnt * 4, cudaMemcpyHostToDevice, h->stream));
+        for (int a = 0; a < 3; ++a)
+            CU_TRY(cudaMemcpyAsync(stg + cnt * (1 + a), u_host + (size_t)h->N * a + plane * z0, cnt * 4,
+                                   cudaMemcpyHostToDevice, h->stream));
+        KParams p = h->kp;
+        p.rho_in = stg; p.u_in = stg + cnt; p.Nio = (long long)cnt; p.zoff = 0;
+        p.z0 = z0; p.z1 = z0 + zc; p.dst = p.src;
+        CU_TRY(launch_init(h, p, zc));
+    }
+    h->t = 0; h->inited = true;
+    int rc = stats_reset_impl(h);
+    if (rc) return rc;
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_step(lbm_t *h, int n)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init / lbm_set_macros");
+    if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
+    for (int k = 0; k < n; ++k) {
+        const bool sample = h->stats_every > 0 && (h->stats_phase % h->stats_every) == 0;
+        KParams p = h->kp;
+        if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
+        if (sample) {
+            p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
+            p.shift = reinterpret_cast<const float *>(h->ws + h->L.shift);
+        }
+        CU_TRY(launch_step(h, p, sample));
+        if (sample) {
+            CU_TRY(launch_stage2(h, 0));
+            h->nsamples++;
+        }
+        if (h->stats_every > 0) h->stats_phase++;
+        h->t++;
+    }
+    return LBM_OK;
+}
+
+// current read-side parameters (two-lattice: the array holding state t)
+static KParams read_params(lbm_s *h)
+{
+    KParams p = h->kp;
+    if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
+    return p;
+}
+
+int lbm_get_macros(lbm_t *h, float *rho_dev, float *u_dev)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_get_macros before lbm_init / lbm_set_macros");
+    KParams p = read_params(h);
+    p.rho_out = rho_dev; p.u_out = u_dev;
+    CU_TRY(launch_macros(h, p, h->nz));
+    return LBM_OK;
+}
+
+int lbm_get_macros_host(lbm_t *h, float *rho_host, float *u_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_get_macros_host before lbm_init / lbm_set_macros");
+    const size_t plane = (size_t)h->nx * h->ny;
+    float *stg = reinterpret_cast<float *>(h->ws + h->L.staging);
+    for (int z0 = 0; z0 < h->nz; z0 += h->L.stage_planes) {
+        const int zc = (h->nz - z0 < h->L.stage_planes) ? h->nz - z0 : h->L.stage_planes;
+        const size_t cnt = plane * zc;
+        KParams p = read_params(h);
+        p.rho_out = rho_host ? stg : nullptr;
+        p.u_out = u_host ? stg + cnt : nullptr;
+        p.Nio = (long long)cnt; p.zoff = 0; p.z0 = z0; p.z1 = z0 + zc;
+        CU_TRY(launch_macros(h, p, zc));
+        if (rho_host)
+            CU_TRY(cudaMemcpyAsync(rho_host + plane * z0, stg, cnt * 4, cudaMemcpyDeviceToHost, h->stream));
+        if (u_host)
+            for (int a = 0; a < 3; ++a)
+                CU_TRY(cudaMemcpyAsync(u_host + (size_t)h->N * a + plane * z0, stg + cnt * (1 + a), cnt * 4,
+                                       cudaMemcpyDeviceToHost, h->stream));
+    }
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_get_state(lbm_t *h, float *out_dev)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_get_state before lbm_init / lbm_set_macros");
+    if (!out_dev) return fail(LBM_EINVAL, "output is NULL");
+    KParams p = read_params(h);
+    const unsigned blocks = (unsigned)((h->N + 255) / 256);
+    if (!h->aa) state_kernel<0><<<blocks, 256, 0, h->stream>>>(p, out_dev);
+    else if (h->t & 1) state_kernel<1><<<blocks, 256, 0, h->stream>>>(p, out_dev);
+    else state_kernel<2><<<blocks, 256, 0, h->stream>>>(p, out_dev);
+    h->launches++;
+    CU_TRY(cudaGetLastError());
+    return LBM_OK;
+}
+
+int lbm_stats_accumulate(lbm_t *h, int every)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (every < 0) return fail(LBM_EINVAL, "every must be >= 0");
+    h->stats_every = every; h->stats_phase = 0;
+    return LBM_OK;
+}
+
+int lbm_stats_reset(lbm_t *h)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_reset before lbm_bind");
+    return stats_reset_impl(h);
+}
+
+int lbm_stats_read(lbm_t *h, double *out, long long *nsamples)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_read before lbm_bind");
+    if (!out) return fail(LBM_EINVAL, "out is NULL");
+    std::vector<double> acc((size_t)h->ny * NSTAT);
+    std::vector<float> shift((size_t)h->ny * 4);
+    int flag = 0;
+    CU_TRY(cudaMemcpyAsync(acc.data(), h->ws + h->L.acc, acc.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaMemcpyAsync(shift.data(), h->ws + h->L.shift, shift.size() * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaMemcpyAsync(&flag, h->ws + h->L.flag, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    if (nsamples) *nsamples = h->nsamples;
+    const double cnt = (double)h->nsamples * h->nx * h->nz;
+    for (int y = 0; y < h->ny; ++y) {
+        const double *a = acc.data() + (size_t)y * NSTAT;
+        double *r = out + (size_t)y * NSTAT;
+        if (h->nsamples == 0) { for (int k = 0; k < NSTAT; ++k) r[k] = 0.0; continue; }
+        // sums are of (u - u0, v - v0, w - w0, rho - 1): second moments about the mean are
+        // shift-invariant, first moments get the centre added back (R18)
+        const double mu = a[0] / cnt, mv = a[1] / cnt, mw = a[2] / cnt;
+        r[0] = mu + shift[y * 4 + 0]; r[1] = mv + shift[y * 4 + 1]; r[2] = mw + shift[y * 4 + 2];
+        r[3] = a[3] / cnt - mu * mu; r[4] = a[4] / cnt - mv * mv; r[5] = a[5] / cnt - mw * mw;
+        r[6] = a[6] / cnt - mu * mv; r[7] = a[7] / cnt - mv * mw; r[8] = a[8] / cnt - mu * mw;
+        r[9] = 1.0 + a[9] / cnt;
+    }
+    if (flag) return fail(LBM_EDIVERGED, "non-finite plane sum of rho seen by the statistics reduction");
+    return LBM_OK;
+}
+
+long long lbm_time(const lbm_t *h) { return h ? h->t : -1; }
+long long lbm_launch_count(const lbm_t *h) { return h ? h->launches : -1; }
+const char *lbm_variant(const lbm_t *h) { return h ? h->variant : ""; }
+
+void lbm_destroy(lbm_t *h) { delete h; }
+
+int lbm_lad_profile(int hc, int ny, double LAI, double eta_m, double *out)
+{
+    if (!out || ny < 1 || hc < 0 || hc > ny) return fail(LBM_EINVAL, "bad lad_profile arguments");
+    if (!(eta_m > 0.0 && eta_m < 1.0)) return fail(LBM_EINVAL, "eta_m must be in (0,1)");
+    double sum = 0.0;
+    for (int j = 0; j < ny; ++j) {
+        double s = 0.0;
+        if (j < hc) {
+            // Eq. 14 (L107) with Eq. 15 (L112): n = 6 below the LAD maximum, 1/2 above
+            const double eta = (j + 0.5) / hc;
+            const double ratio = (1.0 - eta_m) / (1.0 - eta);
+            const double n = (eta < eta_m) ? 6.0 : 0.5;
+            s = std::exp(n * std::log(ratio) + n * (1.0 - ratio));
+        }
+        out[j] = s; sum += s;
+    }
+    for (int j = 0; j < ny; ++j) out[j] = (sum > 0.0) ? out[j] * (LAI / sum) : 0.0;
+    return LBM_OK;
+}
+
+uint64_t lbm_mix64(uint64_t seed, uint64_t ctr) { return lbm::mix64(seed, ctr); }
+

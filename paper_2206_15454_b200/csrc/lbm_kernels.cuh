@@ -1,0 +1,665 @@
+// lbm_kernels.cuh — sm_100a kernels of the fused D3Q19 LES + forest-canopy LBM step.
+//
+// One kernel launch = one time step of Algorithm 1: stream (Eq. 1),
+// moments (Eqs. 5-7), predictor velocity + forest drag + velocity correction (Eq. 6,
+// Eq. 13, Alg. 1), Smagorinsky tau_total (Eqs. 10-12), Guo-forced BGK
+// collision (Eqs. 1-4), boundary links (L177, L216) and the store, with the stage-1
+// x-row sums of the plane statistics (L200, L251) fused into the epilogue.
+//
+// B200 design: HBM-bound stencil, 152 B per cell update.
+//  * populations are fp32 structure-of-arrays, stored SHIFTED (g_i = f_i - w_i) so that fp32
+//    rounding acts on the O(Ma) deviation instead of on the O(1) weights;
+//  * each thread owns V = 4 (2, 1) consecutive x cells: every population row is moved with
+//    aligned 128-bit (64-, 32-bit) loads and stores; the +-1 x shift of 10 of the 19 directions
+//    is done in registers with one warp shuffle, only the two edge lanes of a warp touch one
+//    extra element;
+//  * two storage schemes: two-lattice pull (src -> dst) and the in-place AA pattern (even step
+//    reads/writes its own cell with swapped slots, odd step reads/writes the neighbours), which
+//    halves the memory and makes config 5 (604 M cells) a 46 GB problem;
+//  * boundary rows are handled by per-lane slot/row selection (no divergent shuffles), flags are
+//    a handful of bits in a kernel parameter, the canopy is a per-row table (C_D a_j).
+//
+// This file shares nothing with oracle/ (different arithmetic form: pairwise even/odd
+// collision on shifted populations, fp32).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <type_traits>
+
+namespace lbm {
+
+constexpr int Q = 19;
+constexpr int NSTAT = 10;
+constexpr int MAX_THREADS = 256;
+
+// D3Q19 velocity set in the specification numbering (include/lbm.h).
+struct Lat {
+    static constexpr int cx[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+    static constexpr int cy[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+    static constexpr int cz[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+    static constexpr int opp[Q] = {0, 2, 1, 4, 3, 6, 5, 8, 7, 10, 9, 12, 11, 14, 13, 16, 15, 18, 17};
+    static constexpr int mir[Q] = {0, 1, 2, 4, 3, 5, 6, 9, 10, 7, 8, 11, 12, 13, 14, 18, 17, 16, 15};
+};
+
+// How the streamed (pre-collision) populations of a cell are fetched / how the post-collision
+// ones are put back.
+enum ReadMode { RD_LOCAL = 0,   // A[i][x]                         (AA even step; AA state, t even)
+                RD_PULL = 1,    // A[i][x - c_i]                   (two-lattice)
+                RD_PULL_OPP = 2 // A[opp i][x - c_i]               (AA odd step; AA state, t odd)
+};
+enum WriteMode { WR_LOCAL = 0,     // B[i][x]                      (two-lattice)
+                 WR_LOCAL_OPP = 1, // A[opp i][x]                  (AA even step)
+                 WR_PUSH = 2       // A[i][x + c_i]                (AA odd step, AA init)
+};
+
+enum { BC_BOT_WALL = 0, BC_BOT_PERIODIC = 1 };
+enum { BC_TOP_WALL = 0, BC_TOP_SLIP = 1, BC_TOP_PERIODIC = 2 };
+
+struct KParams {
+    float *src;          // population array read  [19][N]
+    float *dst;          // population array written (== src for AA)
+    int nx, ny, nz;
+    int nchunk;          // blocks per x row
+    long long N;
+    // physics (fp32 copies)
+    float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
+    float Fbx, Fby, Fbz;        // body force density F_b
+    const float *cda;           // [ny] C_D * a_j   (0 = not forest)
+    int bot, top, drag_vector;
+    // statistics
+    float *partial;             // [ny][NSTAT][nz*nchunk]
+    const float *shift;         // [ny][4] accumulation centre (u0, v0, w0, -), may be NULL
+    // macros / init
+    float *rho_out, *u_out;
+    const float *rho_in, *u_in; // init from fields (NULL -> synthetic)
+    const float *uprof;         // [ny] synthetic profile U(y_j)
+    double noise_amp;           // noise_frac * U_ref
+    unsigned long long seed;
+    int z0, z1;                 // z range for chunked host transfers (macros / set_macros)
+    long long zoff;             // element offset of plane z0 inside rho_in/u_in/rho_out/u_out
+    long long Nio;              // component stride of u_in / u_out
+};
+
+// ---------------------------------------------------------------------------------------------
+// small helpers
+// ---------------------------------------------------------------------------------------------
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F &&f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+
+template <int V> __device__ __forceinline__ void ldv(const float *p, float (&o)[V])
+{
+    if constexpr (V == 4) {
+        float4 t = *reinterpret_cast<const float4 *>(p);
+        o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
+    } else if constexpr (V == 2) {
+        float2 t = *reinterpret_cast<const float2 *>(p);
+        o[0] = t.x; o[1] = t.y;
+    } else {
+        o[0] = *p;
+    }
+}
+template <int V> __device__ __forceinline__ void stv(float *p, const float (&o)[V])
+{
+    if constexpr (V == 4) *reinterpret_cast<float4 *>(p) = make_float4(o[0], o[1], o[2], o[3]);
+    else if constexpr (V == 2) *reinterpret_cast<float2 *>(p) = make_float2(o[0], o[1]);
+    else *p = o[0];
+}
+
+// Per-thread geometry: V cells x0..x0+V-1 of row (y, z).
+struct Ctx {
+    int x0, y, z;
+    int xl, xr;        // wrapped x0-1, x0+V
+    int ym, yp, zm, zp; // neighbour rows (wrapped / clamped)
+    bool bot_bb, top_bb, top_fs; // this row touches a wall / free-slip face
+    bool edgeL, edgeR;  // lane has no x-neighbour lane on that side
+};
+
+template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0)
+{
+    Ctx c;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int lane = (ty * blockDim.x + tx) & 31;
+    c.x0 = (blockIdx.y * blockDim.x + tx) * V;
+    const int row = row0 + blockIdx.x * blockDim.y + ty;
+    c.z = row / p.ny;
+    c.y = row - c.z * p.ny;
+    c.xl = (c.x0 == 0) ? p.nx - 1 : c.x0 - 1;
+    c.xr = (c.x0 + V >= p.nx) ? 0 : c.x0 + V;
+    c.zm = (c.z == 0) ? p.nz - 1 : c.z - 1;
+    c.zp = (c.z == p.nz - 1) ? 0 : c.z + 1;
+    const bool isbot = (c.y == 0), istop = (c.y == p.ny - 1);
+    c.ym = isbot ? (p.bot == BC_BOT_PERIODIC ? p.ny - 1 : c.y) : c.y - 1;
+    c.yp = istop ? (p.top == BC_TOP_PERIODIC ? 0 : c.y) : c.y + 1;
+    c.bot_bb = isbot && p.bot == BC_BOT_WALL;
+    c.top_bb = istop && p.top == BC_TOP_WALL;
+    c.top_fs = istop && p.top == BC_TOP_SLIP;
+    c.edgeL = (lane == 0) || (tx == 0);
+    c.edgeR = (lane == 31) || (tx == (int)blockDim.x - 1);
+    return c;
+}
+
+// ---------------------------------------------------------------------------------------------
+// S1: stream.  Fetch the V incoming populations of direction I (Eq. 1 LHS, L41; Alg. 1).
+//   normal link      : slot I      at (x - c_x, y - c_y, z - c_z), periodic wrap in x, z (L177)
+//   wall face        : slot opp(I) at the cell itself (halfway bounce-back; R11, R12)
+//   free-slip face   : slot mir(I) at (x - c_x, y, z - c_z)  (specular reflection; R13)
+// RD_PULL_OPP stores every population in the opposite slot (AA after an even step).
+// ---------------------------------------------------------------------------------------------
+template <int V, int RM, int I>
+__device__ __forceinline__ void load_dir(const KParams &p, const Ctx &c, float (&o)[V])
+{
+    constexpr int cx = Lat::cx[I], cy = Lat::cy[I], cz = Lat::cz[I];
+    if constexpr (RM == RD_LOCAL) {
+        ldv<V>(p.src + (long long)I * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), o);
+        return;
+    } else {
+        constexpr int S_N = (RM == RD_PULL) ? I : Lat::opp[I];
+        constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[I] : I;
+        constexpr int S_FS = (RM == RD_PULL) ? Lat::mir[I] : Lat::opp[Lat::mir[I]];
+        bool bb = false, fs = false;
+        if constexpr (cy == 1) bb = c.bot_bb;
+        if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
+        const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.ym : c.yp);
+        const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zm : c.zp);
+        const int slot = bb ? S_BB : (fs ? S_FS : S_N);
+        const int yrow = (bb || fs) ? c.y : ysel;
+        const int zrow = bb ? c.z : zsel;
+        const float *rowp = p.src + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
+        if constexpr (cx == 0) {
+            ldv<V>(rowp + c.x0, o);
+        } else if constexpr (V == 1) {
+            const int xs = bb ? c.x0 : (cx == 1 ? c.xl : c.xr);
+            o[0] = rowp[xs];
+        } else {
+            float v[V];
+            ldv<V>(rowp + c.x0, v);
+            if constexpr (cx == 1) {           // need x0-1 .. x0+V-2
+                const bool need = c.edgeL && !bb;
+                float e = 0.f;
+                if (need) e = rowp[c.xl];
+                float l = __shfl_up_sync(0xffffffffu, v[V - 1], 1);
+                l = c.edgeL ? e : l;
+                o[0] = bb ? v[0] : l;
+#pragma unroll
+                for (int k = 1; k < V; ++k) o[k] = bb ? v[k] : v[k - 1];
+            } else {                            // need x0+1 .. x0+V
+                const bool need = c.edgeR && !bb;
+                float e = 0.f;
+                if (need) e = rowp[c.xr];
+                float r = __shfl_down_sync(0xffffffffu, v[0], 1);
+                r = c.edgeR ? e : r;
+#pragma unroll
+                for (int k = 0; k < V - 1; ++k) o[k] = bb ? v[k] : v[k + 1];
+                o[V - 1] = bb ? v[V - 1] : r;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S7: store the V post-collision populations of direction I.
+//   WR_LOCAL / WR_LOCAL_OPP : own cell, slot I / opp(I), aligned.
+//   WR_PUSH (AA odd step)   : slot I at (x + c); a link that leaves through a wall face goes to
+//                             slot opp(I) of the own cell, through a free-slip face to slot
+//                             mir(I) at (x + c_x, y, z + c_z) - the places where the next even
+//                             step expects its incoming populations.
+// ---------------------------------------------------------------------------------------------
+template <int V, int WM, int I>
+__device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const float (&r)[V])
+{
+    constexpr int cx = Lat::cx[I], cy = Lat::cy[I], cz = Lat::cz[I];
+    if constexpr (WM != WR_PUSH) {
+        constexpr int S = (WM == WR_LOCAL) ? I : Lat::opp[I];
+        stv<V>(p.dst + (long long)S * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), r);
+        return;
+    } else {
+        bool bb = false, fs = false;
+        if constexpr (cy == -1) bb = c.bot_bb;
+        if constexpr (cy == 1) { bb = c.top_bb; fs = c.top_fs; }
+        const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.yp : c.ym);
+        const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zp : c.zm);
+        constexpr int S_BB = Lat::opp[I], S_FS = Lat::mir[I];
+        const int slot = bb ? S_BB : (fs ? S_FS : I);
+        const int yrow = (bb || fs) ? c.y : ysel;
+        const int zrow = bb ? c.z : zsel;
+        float *rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
+        if constexpr (cx == 0) {
+            stv<V>(rowp + c.x0, r);
+        } else if constexpr (V == 1) {
+            const int xs = bb ? c.x0 : (cx == 1 ? c.xr : c.xl);
+            rowp[xs] = r[0];
+        } else {
+            if constexpr (cx == 1) {           // values land on x0+1 .. x0+V
+                const float l = __shfl_up_sync(0xffffffffu, r[V - 1], 1);
+                if (bb) {
+                    stv<V>(rowp + c.x0, r);
+                } else {
+                    if (!c.edgeL) {
+                        float t[V];
+                        t[0] = l;
+#pragma unroll
+                        for (int k = 1; k < V; ++k) t[k] = r[k - 1];
+                        stv<V>(rowp + c.x0, t);
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < V - 1; ++k) rowp[c.x0 + 1 + k] = r[k];
+                    }
+                    if (c.edgeR) rowp[c.xr] = r[V - 1];
+                }
+            } else {                            // values land on x0-1 .. x0+V-2
+                const float rr = __shfl_down_sync(0xffffffffu, r[0], 1);
+                if (bb) {
+                    stv<V>(rowp + c.x0, r);
+                } else {
+                    if (!c.edgeR) {
+                        float t[V];
+#pragma unroll
+                        for (int k = 0; k < V - 1; ++k) t[k] = r[k + 1];
+                        t[V - 1] = rr;
+                        stv<V>(rowp + c.x0, t);
+                    } else {
+#pragma unroll
+                        for (int k = 1; k < V; ++k) rowp[c.x0 + k - 1] = r[k];
+                    }
+                    if (c.edgeL) rowp[c.xl] = r[0];
+                }
+            }
+        }
+    }
+}
+
+template <int V, int RM>
+__device__ __forceinline__ void load_all(const KParams &p, const Ctx &c, float (&g)[Q][V])
+{
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        load_dir<V, RM, i>(p, c, g[i]);
+    });
+}
+template <int V, int WM>
+__device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, const float (&g)[Q][V])
+{
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        store_dir<V, WM, i>(p, c, g[i]);
+    });
+}
+
+// ---------------------------------------------------------------------------------------------
+// S2-S4: moments of the shifted populations, predictor velocity, forest drag, corrected
+// velocity and total force of one cell (Eqs. 5-7, 13; Alg. 1).
+// Pair sums/differences s_k = g_a + g_b, d_k = g_a - g_b over the 9 opposite pairs feed both the
+// moments and the collision.
+// ---------------------------------------------------------------------------------------------
+struct Cell {
+    float drho, rho, inv_rho;
+    float ux, uy, uz;   // force-corrected velocity (the sample S)
+    float Fx, Fy, Fz;   // total force density F_b + F_f
+    float Pxx, Pyy, Pzz, Pxy, Pyz, Pxz; // sum g_i c c  (= Pi - I/3)
+};
+
+template <int V>
+__device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V], int k, float cda)
+{
+    Cell m;
+    const float s1 = g[1][k] + g[2][k], d1 = g[1][k] - g[2][k];
+    const float s3 = g[3][k] + g[4][k], d3 = g[3][k] - g[4][k];
+    const float s5 = g[5][k] + g[6][k], d5 = g[5][k] - g[6][k];
+    const float s7 = g[7][k] + g[8][k], d7 = g[7][k] - g[8][k];
+    const float s9 = g[9][k] + g[10][k], d9 = g[9][k] - g[10][k];
+    const float s11 = g[11][k] + g[12][k], d11 = g[11][k] - g[12][k];
+    const float s13 = g[13][k] + g[14][k], d13 = g[13][k] - g[14][k];
+    const float s15 = g[15][k] + g[16][k], d15 = g[15][k] - g[16][k];
+    const float s17 = g[17][k] + g[18][k], d17 = g[17][k] - g[18][k];
+    const float sxy = s7 + s9, sxz = s11 + s13, syz = s15 + s17;
+    m.drho = g[0][k] + ((s1 + s3) + (s5 + sxy)) + (sxz + syz);          // Eq. 5 minus 1
+    const float mx = (d1 + d7) + (d9 + d11) + d13;                      // Eq. 6 (bare momentum)
+    const float my = (d3 + d7) + (d15 + d17) - d9;
+    const float mz = (d5 + d11) + (d15 - d13) - d17;
+    m.Pxx = s1 + sxy + sxz;                                              // Eq. 7 minus I/3
+    m.Pyy = s3 + sxy + syz;
+    m.Pzz = s5 + sxz + syz;
+    m.Pxy = s7 - s9;
+    m.Pxz = s11 - s13;
+    m.Pyz = s15 - s17;
+    m.rho = 1.0f + m.drho;
+    m.inv_rho = 1.0f / m.rho;
+    // Alg. 1: local velocity with the driving force (Eq. 6; R7)
+    const float usx = (mx + 0.5f * p.Fbx) * m.inv_rho;
+    const float usy = (my + 0.5f * p.Fby) * m.inv_rho;
+    const float usz = (mz + 0.5f * p.Fbz) * m.inv_rho;
+    float Ffx = 0.f, Ffy = 0.f, Ffz = 0.f;
+    if (cda > 0.f) {
+        // Alg. 1, Eq. 13: F_f = -C_D a_f(y) |u| u, no rho factor (R4), streamwise only (R5)
+        const float mag = sqrtf(usx * usx + usy * usy + usz * usz);
+        const float coef = -cda * mag;
+        Ffx = coef * usx;
+        if (p.drag_vector) { Ffy = coef * usy; Ffz = coef * usz; }
+    }
+    // Alg. 1: correct the velocity with the forest force (explicit; R6)
+    const float hir = 0.5f * m.inv_rho;
+    m.ux = usx + hir * Ffx; m.uy = usy + hir * Ffy; m.uz = usz + hir * Ffz;
+    m.Fx = p.Fbx + Ffx; m.Fy = p.Fby + Ffy; m.Fz = p.Fbz + Ffz;
+    return m;
+}
+
+// S5-S6: Smagorinsky tau_total (Eqs. 10-12; R8, R9) and the forced BGK collision (Eqs. 1-4; R1,
+// R10) in even/odd pair form on the shifted populations:
+//   g*_i = (1-w) g_i + w (f_eq,i - w_i) + F_i,
+//   f_eq,i - w_i = w_i [ drho + rho (3 cu + 4.5 cu^2 - 1.5 uu) ],
+//   F_i = (1 - w/2) w_i [ 3 cF - 3 uF + 9 cu cF ],  w = 1/tau_total.
+template <int V>
+__device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m)
+{
+    const float ux = m.ux, uy = m.uy, uz = m.uz, rho = m.rho;
+    const float third_drho = m.drho * (1.0f / 3.0f);
+    const float nxx = m.Pxx - third_drho - rho * ux * ux;   // Pi_neq = Pi - Pi_eq (L69)
+    const float nyy = m.Pyy - third_drho - rho * uy * uy;
+    const float nzz = m.Pzz - third_drho - rho * uz * uz;
+    const float nxy = m.Pxy - rho * ux * uy;
+    const float nyz = m.Pyz - rho * uy * uz;
+    const float nxz = m.Pxz - rho * ux * uz;
+    const float QQ = (nxx * nxx + nyy * nyy + nzz * nzz) + 2.0f * (nxy * nxy + nyz * nyz + nxz * nxz);
+    const float Qh = sqrtf(QQ);                                                 // Eq. 11
+    const float tau = 0.5f * (p.tau0 + sqrtf(p.tau0sq + p.ksmag * Qh * m.inv_rho)); // Eq. 12
+    const float w = 1.0f / tau;
+    const float omw = 1.0f - w;
+    const float gp = 1.0f - 0.5f * w;                                           // Guo prefactor (R10)
+    const float uu = ux * ux + uy * uy + uz * uz;
+    const float uF = ux * m.Fx + uy * m.Fy + uz * m.Fz;
+    // common even part: w (drho - 1.5 rho uu) - 3 gp uF
+    const float ev0 = w * (m.drho - 1.5f * rho * uu) - 3.0f * gp * uF;
+    const float a2 = 4.5f * w * rho;   // multiplies cu^2
+    const float a1 = 3.0f * w * rho;   // multiplies cu
+    const float b2 = 9.0f * gp;        // multiplies cu cF
+    const float b1 = 3.0f * gp;        // multiplies cF
+    g[0][k] = omw * g[0][k] + (1.0f / 3.0f) * ev0;
+#define LBM_PAIR(A, B, WGT, CU, CF)                                   \
+    {                                                                 \
+        const float cu = (CU), cF = (CF);                             \
+        const float ev = (WGT) * (ev0 + cu * (a2 * cu + b2 * cF));    \
+        const float od = (WGT) * (a1 * cu + b1 * cF);                 \
+        g[A][k] = omw * g[A][k] + (ev + od);                          \
+        g[B][k] = omw * g[B][k] + (ev - od);                          \
+    }
+    LBM_PAIR(1, 2, 1.0f / 18.0f, ux, m.Fx)
+    LBM_PAIR(3, 4, 1.0f / 18.0f, uy, m.Fy)
+    LBM_PAIR(5, 6, 1.0f / 18.0f, uz, m.Fz)
+    LBM_PAIR(7, 8, 1.0f / 36.0f, ux + uy, m.Fx + m.Fy)
+    LBM_PAIR(9, 10, 1.0f / 36.0f, ux - uy, m.Fx - m.Fy)
+    LBM_PAIR(11, 12, 1.0f / 36.0f, ux + uz, m.Fx + m.Fz)
+    LBM_PAIR(13, 14, 1.0f / 36.0f, ux - uz, m.Fx - m.Fz)
+    LBM_PAIR(15, 16, 1.0f / 36.0f, uy + uz, m.Fy + m.Fz)
+    LBM_PAIR(17, 18, 1.0f / 36.0f, uy - uz, m.Fy - m.Fz)
+#undef LBM_PAIR
+}
+
+// ---------------------------------------------------------------------------------------------
+// S8: stage 1 of the plane statistics - x-row sums of the sample S (L200, L251; R18).
+// Columns: u, v, w, uu, vv, ww, uv, vw, uw, rho-1, all about the per-row centre `shift`.
+// The block owns blockDim.y row segments; each is reduced with warp shuffles (+ shared memory
+// across the warps of a segment) and stored, without atomics, to
+//   partial[(y*NSTAT + k) * (nz*nchunk) + z*nchunk + chunk].
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void stats_add(float (&s)[NSTAT], const Cell &m, float u0, float v0, float w0)
+{
+    const float a = m.ux - u0, b = m.uy - v0, c = m.uz - w0;
+    s[0] += a; s[1] += b; s[2] += c;
+    s[3] += a * a; s[4] += b * b; s[5] += c * c;
+    s[6] += a * b; s[7] += b * c; s[8] += a * c;
+    s[9] += m.drho;
+}
+
+__device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c, float (&s)[NSTAT])
+{
+    __shared__ float sred[MAX_THREADS / 32][NSTAT];
+    __shared__ float srow[MAX_THREADS][NSTAT + 1];
+    const int TX = blockDim.x, tx = threadIdx.x, ty = threadIdx.y;
+    const int lin = ty * TX + tx, warp = lin >> 5, lane = lin & 31;
+    const long long pstride = (long long)p.nz * p.nchunk;
+    float *out = p.partial + ((long long)c.y * NSTAT) * pstride + (long long)c.z * p.nchunk + blockIdx.y;
+    if ((TX & 31) == 0) {
+        // every warp lies inside one row segment
+#pragma unroll
+        for (int k = 0; k < NSTAT; ++k) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+        }
+        const int wpr = TX >> 5;
+        if (wpr == 1) {
+            if (lane < NSTAT) {
+                float v = s[0];
+#pragma unroll
+                for (int k = 1; k < NSTAT; ++k) v = (lane == k) ? s[k] : v;
+                out[(long long)lane * pstride] = v;
+            }
+        } else {
+            if (lane == 0) {
+#pragma unroll
+                for (int k = 0; k < NSTAT; ++k) sred[warp][k] = s[k];
+            }
+            __syncthreads();
+            if (tx < NSTAT) {
+                float v = 0.f;
+                for (int q = 0; q < wpr; ++q) v += sred[ty * wpr + q][tx];
+                out[(long long)tx * pstride] = v;
+            }
+        }
+    } else if (TX < 32 && (TX & (TX - 1)) == 0) {
+        // several whole row segments per warp: butterfly inside aligned groups of TX lanes
+#pragma unroll
+        for (int k = 0; k < NSTAT; ++k) {
+            for (int o = TX >> 1; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+        }
+        if (tx == 0) {
+#pragma unroll
+            for (int k = 0; k < NSTAT; ++k) out[(long long)k * pstride] = s[k];
+        }
+    } else {
+        // irregular width: go through shared memory
+#pragma unroll
+        for (int k = 0; k < NSTAT; ++k) srow[lin][k] = s[k];
+        __syncthreads();
+        if (tx < NSTAT) {
+            float v = 0.f;
+            for (int q = 0; q < TX; ++q) v += srow[ty * TX + q][tx];
+            out[(long long)tx * pstride] = v;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The step kernel.  grid = (row blocks, x chunks), block = (TX, TY) <= 256 threads.
+// ---------------------------------------------------------------------------------------------
+template <int V> struct Occ { static constexpr int minb = (V == 4) ? 2 : (V == 2 ? 3 : 4); };
+
+template <int V, int RM, int WM, bool STATS>
+__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const KParams p)
+{
+    const Ctx c = make_ctx<V>(p, 0);
+    float g[Q][V];
+    load_all<V, RM>(p, c, g);
+    const float cda = __ldg(p.cda + c.y);
+    float s[NSTAT];
+    float u0 = 0.f, v0 = 0.f, w0 = 0.f;
+    if constexpr (STATS) {
+#pragma unroll
+        for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
+        if (p.shift) {
+            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c.y);
+            u0 = sh.x; v0 = sh.y; w0 = sh.z;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const Cell m = moments<V>(p, g, k, cda);
+        if constexpr (STATS) stats_add(s, m, u0, v0, w0);
+        collide<V>(p, g, k, m);
+    }
+    store_all<V, WM>(p, c, g);
+    if constexpr (STATS) stats_row_reduce(p, c, s);
+}
+
+// Sample S_k without changing the state (R19): the front half of the step (S1-S4).  Writes
+// rho/u when the pointers are given and the stage-1 sums when p.partial is given.
+// Covers rows [z0*ny, z1*ny).
+template <int V, int RM>
+__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const KParams p)
+{
+    const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
+    float g[Q][V];
+    load_all<V, RM>(p, c, g);
+    const float cda = __ldg(p.cda + c.y);
+    float s[NSTAT];
+#pragma unroll
+    for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
+    float u0 = 0.f, v0 = 0.f, w0 = 0.f;
+    if (p.partial && p.shift) {
+        const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c.y);
+        u0 = sh.x; v0 = sh.y; w0 = sh.z;
+    }
+    float r[V], ux[V], uy[V], uz[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const Cell m = moments<V>(p, g, k, cda);
+        stats_add(s, m, u0, v0, w0);
+        r[k] = m.rho; ux[k] = m.ux; uy[k] = m.uy; uz[k] = m.uz;
+    }
+    const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
+    if (p.rho_out) stv<V>(p.rho_out + off, r);
+    if (p.u_out) {
+        stv<V>(p.u_out + off, ux);
+        stv<V>(p.u_out + p.Nio + off, uy);
+        stv<V>(p.u_out + 2 * p.Nio + off, uz);
+    }
+    if (p.partial) stats_row_reduce(p, c, s);
+}
+
+// splitmix64 output function of seed + (ctr+1)*golden.
+__host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long seed, unsigned long long ctr)
+{
+    unsigned long long z = seed + (ctr + 1ULL) * 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+// State 0 (R17): g_i = f_eq,i(rho, u) - w_i with (rho, u) from the caller's fields or from the
+// synthetic recipe (R16), written in the representation the storage scheme wants
+// (WR_LOCAL: two-lattice; WR_PUSH: AA at even t).  Covers rows [z0*ny, z1*ny).
+template <int V, int WM>
+__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const KParams p)
+{
+    const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
+    float g[Q][V];
+    const long long cell0 = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
+    const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        float rho, ux, uy, uz;
+        if (p.rho_in) {
+            rho = p.rho_in[off + k];
+            ux = p.u_in[off + k]; uy = p.u_in[p.Nio + off + k]; uz = p.u_in[2 * p.Nio + off + k];
+        } else {
+            const unsigned long long cell = (unsigned long long)(cell0 + k);
+            const double inv53 = 1.0 / 9007199254740992.0;
+            const double r0 = (double)(mix64(p.seed, 3ULL * cell + 0ULL) >> 11) * inv53;
+            const double r1 = (double)(mix64(p.seed, 3ULL * cell + 1ULL) >> 11) * inv53;
+            const double r2 = (double)(mix64(p.seed, 3ULL * cell + 2ULL) >> 11) * inv53;
+            rho = 1.0f;
+            ux = (float)((double)p.uprof[c.y] + p.noise_amp * (2.0 * r0 - 1.0));
+            uy = (float)(p.noise_amp * (2.0 * r1 - 1.0));
+            uz = (float)(p.noise_amp * (2.0 * r2 - 1.0));
+        }
+        const float drho = rho - 1.0f;
+        const float uu = ux * ux + uy * uy + uz * uz;
+        const float e0 = drho - 1.5f * rho * uu;
+        g[0][k] = (1.0f / 3.0f) * e0;
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            constexpr float wgt = (i < 7) ? (1.0f / 18.0f) : (1.0f / 36.0f);
+            constexpr float ex = (float)Lat::cx[i], ey = (float)Lat::cy[i], ez = (float)Lat::cz[i];
+            const float cu = ex * ux + ey * uy + ez * uz;
+            g[i][k] = wgt * (e0 + rho * cu * (3.0f + 4.5f * cu));
+        });
+    }
+    store_all<V, WM>(p, c, g);
+}
+
+// Plain "state k" (post-collision, un-streamed) populations out of whatever representation the
+// storage holds: out[i][cell] = g*_i(cell).  One cell per thread (checkpoint / tests only).
+//   two-lattice          : src[i][x]
+//   AA, t odd            : src[opp i][x]
+//   AA, t even (PUSH)    : src[i][x + c_i] with the wall / free-slip redirections of store_dir
+template <int MODE>
+__global__ void state_kernel(const KParams p, float *out)
+{
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= p.N) return;
+    const int x = (int)(cell % p.nx);
+    const long long row = cell / p.nx;
+    const int y = (int)(row % p.ny), z = (int)(row / p.ny);
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
+        constexpr int S_OPP = Lat::opp[i], S_MIR = Lat::mir[i];
+        float v;
+        if constexpr (MODE == 0) v = p.src[(long long)i * p.N + cell];
+        else if constexpr (MODE == 1) v = p.src[(long long)S_OPP * p.N + cell];
+        else {
+            int slot = i, xd = x + cx, yd = y + cy, zd = z + cz;
+            xd = (xd < 0) ? p.nx - 1 : (xd >= p.nx ? 0 : xd);
+            zd = (zd < 0) ? p.nz - 1 : (zd >= p.nz ? 0 : zd);
+            if (yd < 0) {
+                if (p.bot == BC_BOT_PERIODIC) yd = p.ny - 1;
+                else { slot = S_OPP; xd = x; yd = y; zd = z; }
+            } else if (yd >= p.ny) {
+                if (p.top == BC_TOP_PERIODIC) yd = 0;
+                else if (p.top == BC_TOP_SLIP) { slot = S_MIR; yd = y; }
+                else { slot = S_OPP; xd = x; yd = y; zd = z; }
+            }
+            v = p.src[(long long)slot * p.N + ((long long)(yd + p.ny * zd) * p.nx + xd)];
+        }
+        out[(long long)i * p.N + cell] = v;
+    });
+}
+
+// ---------------------------------------------------------------------------------------------
+// S9: stage 2 of the statistics - reduce the row partials of one (y, k) over z (and x chunks)
+// in fp64 with warp shuffles + shared memory and add into the running sums acc[y][k].
+// grid = (ny, NSTAT), block = 256.  mode 0: accumulate; mode 1: prime the accumulation centre
+// shift[y][0..2] with the current plane means instead.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) stats_stage2_kernel(const float *__restrict__ partial, long long len,
+                                                           double *acc, float *shift, int mode,
+                                                           double inv_count, int *diverged)
+{
+    __shared__ double sm[8];
+    const int y = blockIdx.x, k = blockIdx.y;
+    const float *src = partial + ((long long)y * NSTAT + k) * len;
+    double t = 0.0;
+    for (long long q = threadIdx.x; q < len; q += blockDim.x) t += (double)src[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) tot += sm[w];
+        if (mode == 0) {
+            acc[y * NSTAT + k] += tot;
+            if (k == NSTAT - 1 && !isfinite(tot)) *diverged = 1;
+        } else if (k < 3) {
+            const double mean = tot * inv_count;
+            shift[y * 4 + k] = isfinite(mean) ? (float)mean : 0.f;
+        }
+    }
+}
+
+} // namespace lbm

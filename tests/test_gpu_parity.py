@@ -1,0 +1,298 @@
+"""GPU-vs-oracle parity of the CUDA path, through the C ABI (pin P10 of DESIGN.md).
+
+Every test runs the CUDA library (paper_2206_15454_b200) and the fp64 CPU oracle (oracle/) on the
+same seeded inputs and compares element by element.  Tolerances:
+  * macroscopic rho, u after <= 200 steps: max|delta| <= 1e-5 * u_bulk (BASELINE.json:north_star);
+  * one-step / few-step population checks: 2e-7 absolute (fp32 rounding of O(0.05) deviations
+    from the weights, a few operations deep), far below any indexing or boundary-link mistake,
+    which shows up at the 1e-3 level.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_REL = 1e-5  # north_star: relative to the bulk velocity
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    lb.lib()
+    return lb
+
+
+def _weights(orc):
+    _, w, _, _ = orc.tables()
+    return w
+
+
+def _pair(orc, gpu, cfg, aa, vec, seed=None):
+    cfg = dict(cfg)
+    if seed is not None:
+        cfg["seed"] = seed
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    g = gpu.Lbm.from_config(cfg, aa=aa, vec=vec)
+    g.init(cfg["seed"])
+    return o, g
+
+
+def _macro_err(o, g):
+    import torch
+    ro, uo = o.get_macros()
+    rg, ug = g.get_macros()
+    torch.cuda.synchronize()
+    rg = rg.cpu().numpy().astype(np.float64)
+    ug = ug.cpu().numpy().astype(np.float64)
+    return float(np.abs(rg - ro).max()), float(np.abs(ug - uo).max())
+
+
+def _state_err(o, g, w):
+    import torch
+    fo = o.get_populations() - w[:, None, None, None]
+    fg = g.get_state()
+    torch.cuda.synchronize()
+    return float(np.abs(fg.cpu().numpy().astype(np.float64) - fo).max())
+
+
+# ---------------------------------------------------------------------------------------------
+# small lattices: every storage scheme x vector width x boundary set, ragged widths
+# ---------------------------------------------------------------------------------------------
+BCS = [(wl.BOUNCE_BACK, wl.FREE_SLIP), (wl.BOUNCE_BACK, wl.BOUNCE_BACK), (wl.PERIODIC, wl.PERIODIC)]
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("nx,vec", [(32, 4), (32, 2), (32, 1), (36, 4), (34, 2), (33, 1), (128, 4),
+                                    (256, 4), (4, 4), (2, 2), (1, 1), (200, 4), (1536, 4)])
+@pytest.mark.parametrize("bottom,top", BCS, ids=["wall-slip", "wall-wall", "periodic"])
+def test_small_state_and_macros(orc, gpu, aa, nx, vec, bottom, top):
+    ny, nz = (6, 3) if nx >= 1024 else (12, 6)
+    cfg = wl.small(nx=nx, ny=ny, nz=nz, bottom=bottom, top=top, drag_vector=False)
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    assert f"v{vec}" in g.variant and (("aa" in g.variant) == aa)
+    assert _state_err(o, g, w) <= 2e-8            # state 0
+    er, eu = _macro_err(o, g)
+    assert er <= 2e-7 and eu <= 2e-8
+    for k in (1, 1, 1, 2, 5):                     # both AA parities, odd and even step counts
+        o.step(k)
+        g.step(k)
+        assert g.time == o.time
+        assert _state_err(o, g, w) <= 2e-7
+        er, eu = _macro_err(o, g)
+        assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+def test_vector_drag_and_general_force(orc, gpu, aa):
+    cfg = wl.small(nx=64, ny=10, nz=8, drag_vector=True)
+    cfg["body_force"] = (2e-6, -1e-6, 5e-7)
+    o, g = _pair(orc, gpu, cfg, aa, 4)
+    w = _weights(orc)
+    o.step(7)
+    g.step(7)
+    assert _state_err(o, g, w) <= 2e-7
+
+
+def test_single_block_shapes(orc, gpu):
+    """Different thread-block shapes (row split across blocks, several rows per block) agree."""
+    cfg = wl.small(nx=256, ny=8, nz=4)
+    w = _weights(orc)
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    o.stats_accumulate(1)
+    o.step(4)
+    so, _ = o.stats_read()
+    for aa in (False, True):
+        for tx, ty in [(64, 1), (32, 2), (16, 4), (8, 8), (64, 4), (32, 8)]:
+            g = gpu.Lbm.from_config(cfg, aa=aa, vec=4)
+            g.set_launch_shape(tx, ty)
+            g.init(cfg["seed"])
+            g.stats_accumulate(1)
+            g.step(4)
+            assert _state_err(o, g, w) <= 2e-7, (aa, tx, ty)
+            sg, n = g.stats_read()
+            assert n == 4
+            _check_stats(sg, so, cfg["u_bulk"])
+
+
+# ---------------------------------------------------------------------------------------------
+# statistics (S8, S9) against the oracle's O10 on identical samples
+# ---------------------------------------------------------------------------------------------
+def _check_stats(sg, so, u_bulk):
+    # means: relative to u_bulk; second moments: relative to u_bulk^2 (fp32 x-row sums, fp64 beyond)
+    assert np.abs(sg[:, 0:3] - so[:, 0:3]).max() <= 1e-5 * u_bulk
+    assert np.abs(sg[:, 3:9] - so[:, 3:9]).max() <= 1e-5 * u_bulk ** 2
+    assert np.abs(sg[:, 9] - so[:, 9]).max() <= 1e-6
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2), (33, 1), (512, 4)])
+def test_stats_parity(orc, gpu, aa, nx, vec):
+    cfg = wl.small(nx=nx, ny=10, nz=6)
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    o.step(3)
+    g.step(3)
+    o.stats_accumulate(2)
+    g.stats_accumulate(2)
+    g.stats_reset()
+    o.stats_reset()
+    o.step(9)
+    g.step(9)
+    so, no = o.stats_read()
+    sg, ng = g.stats_read()
+    assert no == ng == 5
+    _check_stats(sg, so, cfg["u_bulk"])
+    # switching sampling off keeps the sums
+    g.stats_accumulate(0)
+    g.step(2)
+    sg2, ng2 = g.stats_read()
+    assert ng2 == 5 and np.array_equal(sg2, sg)
+
+
+def test_set_macros_host_and_get_macros_host(orc, gpu):
+    import torch
+    cfg = wl.small(nx=64, ny=10, nz=12)
+    o = orc.Oracle.from_config(cfg)
+    rho, u = o.init_field(cfg["init"]["kind"], cfg["init"]["U_ref"], cfg["init"]["noise_frac"], 777)
+    rho = rho * (1.0 + 0.01 * np.sin(np.arange(rho.size).reshape(rho.shape)))
+    o.set_macros(rho, u)
+    w = _weights(orc)
+    for aa in (False, True):
+        g = gpu.Lbm.from_config(cfg, aa=aa)
+        g.set_macros_host(rho.astype(np.float32), u.astype(np.float32))
+        assert _state_err(o, g, w) <= 5e-8
+        g2 = gpu.Lbm.from_config(cfg, aa=aa)
+        g2.set_macros(torch.from_numpy(rho.astype(np.float32)).cuda(), torch.from_numpy(u.astype(np.float32)).cuda())
+        assert _state_err(o, g2, w) <= 5e-8
+        g.step(3)
+        rh, uh = g.get_macros_host()
+        rd, ud = g.get_macros()
+        assert np.array_equal(rh, rd.cpu().numpy()) and np.array_equal(uh, ud.cpu().numpy())
+
+
+# ---------------------------------------------------------------------------------------------
+# config 1 (BASELINE.json:configs[0]) at 1, 10, 100, 200 steps; config 2 at 100 steps
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+def test_cfg1_200_steps(orc, gpu, aa):
+    cfg = wl.get("cfg1")
+    o, g = _pair(orc, gpu, cfg, aa, 0)
+    o.stats_accumulate(1)
+    g.stats_accumulate(1)
+    tol = TOL_REL * cfg["u_bulk"]
+    done = 0
+    for target in (1, 10, 100, 200):
+        o.step(target - done)
+        g.step(target - done)
+        done = target
+        er, eu = _macro_err(o, g)
+        print(f"cfg1 {g.variant} step {target}: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
+        assert er <= tol and eu <= tol
+    so, no = o.stats_read()
+    sg, ng = g.stats_read()
+    assert no == ng == 200
+    _check_stats(sg, so, cfg["u_bulk"])
+    # mass conservation on the GPU side (invariant, any size)
+    assert abs(sg[:, 9].mean() - 1.0) < 1e-6
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+def test_cfg2_100_steps(orc, gpu, aa):
+    cfg = wl.get("cfg2")
+    o, g = _pair(orc, gpu, cfg, aa, 0)
+    tol = TOL_REL * cfg["u_bulk"]
+    o.step(100)
+    g.step(100)
+    er, eu = _macro_err(o, g)
+    print(f"cfg2 {g.variant} step 100: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
+    assert er <= tol and eu <= tol
+
+
+# ---------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times: sampled sub-boxes the oracle
+# can recompute one step at a time + invariants
+# ---------------------------------------------------------------------------------------------
+def _subbox_check(orc, gpu, cfg, aa, boxes, presteps):
+    """Take GPU state k, cut sub-boxes out of it, let the oracle advance each box one step and
+    compare with the GPU's state k+1 on the cells whose neighbours all lie inside the box."""
+    import torch
+    w = _weights(orc)
+    g = gpu.Lbm.from_config(cfg, aa=aa)
+    g.init(cfg["seed"])
+    g.step(presteps)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    lad = gpu.lad_from_spec(cfg["forest"], ny)
+    lad_o = orc.lad_from_spec(cfg["forest"], ny)
+    if lad is not None:
+        assert np.abs(lad - lad_o).max() <= 1e-14
+    S = 8
+
+    def cut(state, x0, y0, z0):
+        xi = torch.arange(x0, x0 + S, device=state.device) % nx
+        zi = torch.arange(z0, z0 + S, device=state.device) % nz
+        sub = state[:, zi][:, :, y0:y0 + S][:, :, :, xi]
+        return sub.cpu().numpy().astype(np.float64)
+
+    st = g.get_state()
+    before = [cut(st, *b) for b in boxes]
+    del st
+    g.step(1)
+    st = g.get_state()
+    after = [cut(st, *b) for b in boxes]
+    del st
+    torch.cuda.synchronize()
+    worst = 0.0
+    for (x0, y0, z0), fb, fa in zip(boxes, before, after):
+        bottom = wl.BOUNCE_BACK
+        top = cfg["top"] if y0 + S == ny else wl.BOUNCE_BACK
+        o = orc.Oracle(S, S, S, cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                       None if lad_o is None else lad_o[y0:y0 + S], orc.bc_flags(bottom, top))
+        o.set_populations(fb + w[:, None, None, None])
+        o.step(1)
+        fo = o.get_populations() - w[:, None, None, None]
+        ylo = 0 if y0 == 0 else 1                 # real wall rows are exact, cut faces are not
+        yhi = S if y0 + S == ny else S - 1
+        d = np.abs(fa - fo)[:, 1:S - 1, ylo:yhi, 1:S - 1]
+        worst = max(worst, float(d.max()))
+    return worst, g
+
+
+@pytest.mark.parametrize("name,aa", [("cfg3", False), ("cfg3", True), ("cfg4", True), ("cfg5", True)])
+def test_full_size_sampled_boxes(orc, gpu, name, aa):
+    import torch
+    cfg = wl.get(name)
+    free, _ = torch.cuda.mem_get_info()
+    need = 76 * wl.n_cells(cfg) * (2 if aa else 3) * 1.05
+    if free < need:
+        pytest.skip(f"{name} needs {need / 2**30:.0f} GiB of device memory")
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    h = cfg["forest"]["h"]
+    boxes = [(0, 0, 0), (nx - 4, 0, nz - 4), (nx // 2 - 3, h - 4, nz // 3), (nx - 8, ny - 8, 0),
+             (5, ny - 8, nz - 5), (nx // 3, ny // 2, nz // 2), (124, 0, 1), (nx - 5, ny // 4, nz - 3)]
+    for presteps in (2, 3):                       # AA: next step is even / odd
+        worst, g = _subbox_check(orc, gpu, cfg, aa, boxes, presteps)
+        print(f"{name} {g.variant} presteps={presteps}: worst one-step |delta f| = {worst:.3e}")
+        assert worst <= 2e-7
+        # invariant at any size: mass is conserved (rho plane means average to 1)
+        g.stats_accumulate(1)
+        g.stats_reset()
+        g.step(2)
+        s, n = g.stats_read()
+        assert n == 2 and abs(s[:, 9].mean() - 1.0) < 2e-6
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+
+
+def test_step_before_init_is_an_error(gpu):
+    g = gpu.Lbm(8, 4, 4, 0.01, 0.1)
+    with pytest.raises(gpu.LbmError) as e:
+        g.step(1)
+    assert e.value.code == gpu.LBM_ESTATE

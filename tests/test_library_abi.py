@@ -1,0 +1,128 @@
+"""CPU-side checks of the CUDA library: it builds for sm_100a, loads, exports every symbol that
+include/lbm.h declares, and its host-only entry points behave (no kernel is launched here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def lb():
+    import paper_2206_15454_b200 as lb
+    lb.lib()
+    return lb
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lbm_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lb):
+    names = _declared_symbols()
+    assert len(names) >= 20
+    L = lb.lib()
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/lbm.h but not exported"
+    assert sorted(lb.SYMBOLS) == names
+
+
+def test_sass_is_sm100a_only():
+    import subprocess
+    from paper_2206_15454_b200 import build
+    out = subprocess.run(["cuobjdump", "-lelf", build.build()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out and not re.search(r"sm_(?!100a)\d+", out)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2206_15454_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), f
+                assert "lbm_oracle" not in src, f
+
+
+def test_create_argument_errors(lb):
+    L = lb.lib()
+    h = C.c_void_p()
+    bf = (C.c_double * 3)(0, 0, 0)
+    dp = C.POINTER(C.c_double)
+
+    def create(nx=8, ny=8, nz=8, nu=0.01, Cs=0.1, Cd=0.0, lad=None, flags=0):
+        return L.lbm_create(C.byref(h), nx, ny, nz, nu, Cs, C.cast(bf, dp), Cd, lad, flags)
+
+    assert create() == lb.LBM_OK
+    L.lbm_destroy(h)
+    assert create(nu=0.0) == lb.LBM_EINVAL and b"nu" in L.lbm_last_error()
+    assert create(nx=0) == lb.LBM_EINVAL
+    assert create(nx=4096, ny=1024, nz=1024) == lb.LBM_EINVAL          # >= 2^31 cells
+    assert create(flags=lb.BOTTOM_PERIODIC | lb.TOP_WALL) == lb.LBM_EINVAL  # periodic-y needs both
+    assert create(flags=3 << 2) == lb.LBM_EINVAL                        # forced-eq top: not built
+    assert create(nx=6, flags=4 << 8) == lb.LBM_EINVAL                  # vec=4 does not divide 6
+    assert create(flags=1 << 20) == lb.LBM_EINVAL
+    bad = (C.c_double * 8)(*([0.1] * 7 + [-1.0]))
+    assert create(lad=C.cast(bad, dp)) == lb.LBM_EINVAL
+    # calls out of order never touch the GPU
+    assert create() == lb.LBM_OK
+    assert L.lbm_step(h, 1) == lb.LBM_ESTATE
+    assert L.lbm_init(h, 1) == lb.LBM_ESTATE
+    assert L.lbm_bind(h, None, 0, None) == lb.LBM_EINVAL
+    assert L.lbm_bind(h, C.c_void_p(256), 16, None) == lb.LBM_ENOMEM
+    L.lbm_destroy(h)
+
+
+def test_workspace_bytes(lb):
+    n = 64 * 32 * 32
+    two = lb.workspace_bytes(64, 32, 32, 0)
+    aa = lb.workspace_bytes(64, 32, 32, lb.STORAGE_AA)
+    assert two - aa == 76 * n                     # the second lattice
+    assert aa >= 76 * n and aa < 76 * n + 16 * n + (4 << 20)
+    # config 5 as an AA single array is a ~46 GB problem (BASELINE.json:configs[4])
+    big = lb.workspace_bytes(1536, 384, 1024, lb.STORAGE_AA)
+    assert 45.9e9 < big < 47.0e9
+
+
+def test_mix64_known_answers(lb):
+    """The library's own counter-based generator against the published splitmix64 vectors."""
+    for line in open(os.path.join(GOLD, "splitmix64_vectors.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        seed, n, val = (int(t) for t in line.split())
+        assert lb.mix64(seed, n) == val
+
+
+def test_lad_profile_closed_forms(lb):
+    """Eqs. 14-15: peak value 1 at eta_m, zero above h, sum = LAI, and the
+    midpoint mean of the shape tends to the quadrature value 0.4601."""
+    for h, ny in [(16, 128), (32, 256), (48, 384)]:
+        a = lb.lad_profile(h, ny, 2.0, 0.7)
+        assert a.shape == (ny,) and np.all(a[h:] == 0) and np.all(a[:h] > 0)
+        assert abs(a.sum() - 2.0) < 1e-12
+        j = int(np.argmax(a))
+        assert abs((j + 0.5) / h - 0.7) <= 0.5 / h + 1e-12
+        eta = (np.arange(h) + 0.5) / h
+        r = 0.3 / (1 - eta)
+        n = np.where(eta < 0.7, 6.0, 0.5)
+        shape = r ** n * np.exp(n * (1 - r))
+        assert np.allclose(a[:h], 2.0 * shape / shape.sum(), rtol=1e-12)
+        assert abs(shape.mean() - 0.4601) < 2e-3
+    # peak a_fm for LAI = 2: 0.2726 (h=16), 0.1358 (h=32), 0.0906 (h=48)
+    assert abs(lb.lad_profile(16, 128, 2.0).max() - 0.2726) < 2e-3
+    assert abs(lb.lad_profile(32, 256, 2.0).max() - 0.1358) < 1e-3
+    assert abs(lb.lad_profile(48, 384, 2.0).max() - 0.0906) < 1e-3
+
+
+def test_no_cpu_fallback(lb):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        lb.Lbm(8, 8, 8, 0.01, 0.1)
