@@ -466,10 +466,10 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
 #pragma unroll
         for (int k = 0; k < NSTAT; ++k) srow[lin][k] = s[k];
         __syncthreads();
-        if (tx < NSTAT) {
+        for (int k = tx; k < NSTAT; k += TX) {   // TX may be smaller than NSTAT
             float v = 0.f;
-            for (int q = 0; q < TX; ++q) v += srow[ty * TX + q][tx];
-            out[(long long)tx * pstride] = v;
+            for (int q = 0; q < TX; ++q) v += srow[ty * TX + q][k];
+            out[(long long)k * pstride] = v;
         }
     }
 }
