@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS and DRAM roofline fraction of the fused D3Q19 LES + forest LBM step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg5] [--impl b200|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one time step of the whole hot path: one fused step-kernel
+launch plus, on the configs that accumulate statistics every step, the stage-2 reduction launch.
+The default workload is BASELINE.json:configs[4] ("cfg5", 1536x384x1024, single-array AA storage,
+45.9 GB of populations), the largest configuration, on which north_star states its target.
+
+One JSON line is printed by rank 0:
+  value        MLUPS (1e6 lattice-cell updates per second), whole job, state resident in HBM
+  e2e          the same metric through the C ABI with HOST buffers: lbm_set_macros_host (pinned
+               host rho,u -> device) + K x [lbm_step(1) + lbm_stats_read (device -> host)]
+  roofline     step kernel only: 152 B/cell x cells / mean device time of the step-kernel launches
+               (CUDA events recorded by the library on its launch stream, lbm_set_kernel_timing)
+               against MEASURED_PEAKS.json's hbm_gbs
+  cpu_baseline the fp64 oracle, as it stands, on the host cores on a bounded slab of the workload
+--gpus N > 1: the path is built for one GPU (replicas only); every rank
+runs an independent replica of the workload and `value` is the sum over replicas.
+--impl reference times the oracle alone (the reference arm of this tier).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star)
+METRIC = "MLUPS"
+UNIT = "MLUPS (1e6 lattice-cell updates/s)"
+
+
+def measured_peak():
+    """HBM copy peak from MEASURED_PEAKS.json (driver-written), else the guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop_flag = threading.Event()
+        self.sm, self.reasons, self.sm_max, self.power = [], set(), None, []
+        self.err = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            }
+            while not self.stop_flag.is_set():
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                except Exception:
+                    pass
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.stop_flag.wait(0.1)
+        except Exception as e:  # NVML missing: report it, do not fail the bench
+            self.err = repr(e)
+
+    def result(self):
+        self.stop_flag.set()
+        self.join(timeout=2.0)
+        sm = sorted(self.sm)
+        out = {"sm_mhz": (sm[len(sm) // 2] if sm else None), "sm_max_mhz": self.sm_max,
+               "reasons": sorted(self.reasons), "samples": len(sm)}
+        if self.power:
+            out["power_w_max"] = round(max(self.power), 1)
+        if self.err:
+            out["error"] = self.err
+        return out
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline of the default arm; the whole of --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample_config(cfg: dict, max_nx: int = 256, max_nz: int = 64) -> dict:
+    """Bounded sample of the workload for the CPU oracle: the same physics, boundary set, canopy
+    table and full wall-normal extent ny, on an x-z sub-slab (periodic) of at most 256 x 64
+    columns, so that the fp64 two-lattice oracle (304 B/cell) stays near 2 GB."""
+    s = dict(cfg)
+    s["nx"] = min(cfg["nx"], max_nx)
+    s["nz"] = min(cfg["nz"], max_nz)
+    return s
+
+
+def time_oracle(cfg: dict, steps: int, warmup: int, budget_s: float = 15.0, max_nx: int = 256,
+                max_nz: int = 64):
+    """Time the oracle as it stands on the host cores.  `steps` = 0: as many steps as fit the
+    time budget (at least 2).  Returns (MLUPS, ms per step, steps, cores, sample text)."""
+    import oracle
+
+    s = oracle_sample_config(cfg, max_nx, max_nz)
+    cores = os.cpu_count() or 1
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except Exception:
+        pass
+    env_threads = os.environ.get("OMP_NUM_THREADS")
+    if env_threads:
+        cores = min(cores, int(env_threads))
+    o = oracle.Oracle.from_config(s)
+    o.init_from_config(s)
+    if s.get("stats_every", 0) > 0:
+        o.stats_accumulate(s["stats_every"])
+    n_cells = wl.n_cells(s)
+    t0 = time.perf_counter()
+    o.step(max(1, warmup))
+    per = (time.perf_counter() - t0) / max(1, warmup)
+    if steps <= 0:
+        steps = int(max(2, min(500, budget_s / max(per, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    o.stats_read()
+    mlups = n_cells * steps / dt / 1e6
+    sample = (f"{s['nx']}x{s['ny']}x{s['nz']} periodic x-z sub-slab of {cfg['name']} "
+              f"({n_cells} cells, same physics/BCs/canopy, full ny), {steps} oracle steps, "
+              f"fp64 two-lattice, gcc -O2 -fopenmp")
+    return mlups, dt / steps * 1e3, steps, cores, sample
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle alone, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    steps = args.steps
+    # bounded sample: each step is one oracle time step of a 128 x ny x 32 slab (~0.3 s)
+    mlups, ms, steps_done, cores, sample = time_oracle(cfg, steps, args.warmup, max_nx=128, max_nz=32)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": round(mlups, 3), "unit": UNIT,
+        "n_gpus": args.gpus, "steps": steps_done, "warmup": args.warmup,
+        "ms_per_step": round(ms, 4), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args, None),
+        "cpu_baseline": {"value": round(mlups, 3), "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": round(mlups, 3), "unit": UNIT, "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(cfg, args, variant):
+    pops_gb = wl.n_cells(cfg) * 76 * (1 if cfg["storage"] == "aa" else 2) / 1e9
+    c = {
+        "workload": f"{cfg['name']}: {cfg['note']}",
+        "lattice": [cfg["nx"], cfg["ny"], cfg["nz"]], "cells": wl.n_cells(cfg),
+        "storage": cfg["storage"], "stats_every": cfg.get("stats_every", 0),
+        "bottom": cfg["bottom"], "top": cfg["top"], "nu": cfg["nu"], "Cs": cfg["Cs"],
+        "Cd": cfg["Cd"], "seed": cfg["seed"],
+        "l2": f"no flush: populations are {pops_gb:.2f} GB per pass, larger than the 126 MB L2"
+              if pops_gb > 0.2 else "L2-resident workload (populations fit the 126 MB L2): "
+              "the DRAM roofline fraction is not meaningful here",
+        "parallelism": "1 GPU" if args.gpus == 1 else f"{args.gpus} independent replicas",
+    }
+    if variant:
+        c["kernel_variant"] = variant
+    return c
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA leg
+# ---------------------------------------------------------------------------------------------
+def run_b200(args, cfg):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_2206_15454_b200 as lb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, W = args.steps, args.warmup
+    N = wl.n_cells(cfg)
+    aa = cfg["storage"] == "aa"
+    every = cfg.get("stats_every", 0)
+    sim = lb.Lbm.from_config(cfg, aa=aa, device=dev)
+    if args.shape:
+        tx, ty = (int(v) for v in args.shape.split("x"))
+        sim.set_launch_shape(tx, ty)
+    sim.init(cfg["seed"] + rank)
+    sim.stats_accumulate(every)
+    stream = torch.cuda.current_stream(dev)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps ----
+    sim.step(W)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    barrier()
+    launches = sim.launch_count - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.result()
+    stats, nsamp = sim.stats_read()
+    if every > 0 and (nsamp != (W + K) // every or not np.isfinite(stats).all()):
+        raise RuntimeError(f"statistics check failed: nsamples={nsamp}, finite={np.isfinite(stats).all()}")
+
+    # ---- roofline leg: the step kernel alone, bracketed per launch by the library ----
+    sim.set_kernel_timing(True)
+    nk = min(K, 4096)
+    sim.step(nk)
+    k_ms, k_n = sim.kernel_timing_read()
+    sim.set_kernel_timing(False)
+    kernel_ms = k_ms / max(1, k_n)
+
+    # ---- end to end through the C ABI with host buffers ----
+    rho_h = torch.empty(sim.shape, dtype=torch.float32).pin_memory()
+    u_h = torch.empty((3,) + sim.shape, dtype=torch.float32).pin_memory()
+    sim.get_macros_host(rho_h, u_h)          # a valid field to restart from (untimed)
+    e2e_steps = K
+    barrier()
+    t0 = time.perf_counter()
+    sim.set_macros_host(rho_h, u_h)          # H2D of the step inputs, then f = f_eq(rho, u)
+    sim.stats_accumulate(max(1, every))
+    out = None
+    for _ in range(e2e_steps):
+        sim.step(1)
+        out, _n = sim.stats_read()           # D2H of the step's result; synchronises
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if not np.isfinite(out).all():
+        raise RuntimeError("end-to-end leg produced non-finite statistics")
+    h2d = (rho_h.numel() + u_h.numel()) * 4 / e2e_steps
+    d2h = cfg["ny"] * (lb.NSTAT * 8 + 16) + 4
+
+    # ---- max over ranks, sum of work ----
+    times = torch.tensor([ms, e2e_s * 1e3, kernel_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    ms, e2e_ms, kernel_ms = (float(v) for v in times.cpu())
+    variant = sim.variant
+    sim.close()
+    del sim, rho_h, u_h
+    torch.cuda.empty_cache()
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        mlups = world * N * K / (ms * 1e-3) / 1e6
+        e2e_mlups = world * N * e2e_steps / (e2e_ms * 1e-3) / 1e6
+        achieved = BYTES_PER_CELL * N / (kernel_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": round(mlups, 1), "unit": UNIT, "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": round(ms / K, 5), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(cfg, args, variant),
+            "algorithmic_gbs": round(mlups * BYTES_PER_CELL / 1e3 / world, 1),
+            "frac_of_nominal_8tbs": round(mlups * BYTES_PER_CELL / 1e3 / world / 8000.0, 4),
+            "roofline": {"bound": "hbm", "kernel": "lbm::step_kernel (" + variant + ")",
+                         "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                         "frac": round(achieved / peak, 4), "traffic": args.traffic,
+                         "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL,
+                         "kernel_ms": round(kernel_ms, 5), "launches_timed": k_n},
+            "e2e": {"value": round(e2e_mlups, 1), "unit": UNIT,
+                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "steps": e2e_steps,
+                    "what": "lbm_set_macros_host(pinned rho,u) + steps x [lbm_step(1) + lbm_stats_read]"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+        }
+        if not args.no_cpu and world == 1:
+            cm, _cms, _cs, cores, sample = time_oracle(cfg, 0, 1)
+            line["cpu_baseline"] = {"value": round(cm, 2), "unit": UNIT, "cores": cores,
+                                    "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
+    ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 (BASELINE.json:configs[0..4])")
+    ap.add_argument("--storage", choices=["aa", "two_lattice"], default=None,
+                    help="override the config's storage scheme")
+    ap.add_argument("--stats-every", type=int, default=None, help="override the config's stats cadence")
+    ap.add_argument("--shape", default=None, help="thread-block shape override TXxTY (tuning)")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="ncu dram bytes (read+write) per step-kernel launch, from profiles/, to quote in the line")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    cfg = wl.get(args.config)
+    if args.storage:
+        cfg["storage"] = args.storage
+    if args.stats_every is not None:
+        cfg["stats_every"] = args.stats_every
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    return run_b200(args, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

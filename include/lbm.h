@@ -141,6 +141,14 @@ long long lbm_launch_count(const lbm_t *h);
  * the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
 
+/* Measurement hook (bench.py "roofline"): with on != 0, lbm_step brackets every step-kernel
+ * launch (the fused S1-S8 kernel only, not the stage-2 reduction) with a pair of CUDA events on
+ * the bound stream, up to 4096 launches between reads.  lbm_kernel_timing_read synchronises the
+ * stream, returns the summed device time of the bracketed launches in milliseconds and their
+ * count, and clears the record.  Either output may be NULL. */
+int lbm_set_kernel_timing(lbm_t *h, int on);
+int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches);
+
 /* Name of the kernel variant lbm_step uses, e.g. "aa/v4/tx384x1" (static string per handle). */
 const char *lbm_variant(const lbm_t *h);
 

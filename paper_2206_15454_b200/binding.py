@@ -34,7 +34,7 @@ SYMBOLS = [
     "lbm_set_macros_host", "lbm_step", "lbm_get_macros", "lbm_get_macros_host",
     "lbm_stats_accumulate", "lbm_stats_read", "lbm_stats_reset", "lbm_get_state", "lbm_time",
     "lbm_launch_count", "lbm_set_launch_shape", "lbm_variant", "lbm_destroy", "lbm_last_error",
-    "lbm_lad_profile", "lbm_mix64",
+    "lbm_lad_profile", "lbm_mix64", "lbm_set_kernel_timing", "lbm_kernel_timing_read",
 ]
 
 
@@ -80,6 +80,8 @@ def lib():
         L.lbm_destroy.restype = None
         L.lbm_last_error.restype = C.c_char_p
         L.lbm_lad_profile.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
+        L.lbm_set_kernel_timing.argtypes = [vp, C.c_int]
+        L.lbm_kernel_timing_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.lbm_mix64.argtypes = [C.c_uint64, C.c_uint64]
         L.lbm_mix64.restype = C.c_uint64
         _lib = L
@@ -279,6 +281,16 @@ class Lbm:
         n = C.c_longlong(0)
         _check(lib().lbm_stats_read(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
         return out, int(n.value)
+
+    def set_kernel_timing(self, on: bool):
+        _check(lib().lbm_set_kernel_timing(self._h, int(bool(on))))
+
+    def kernel_timing_read(self):
+        """(summed step-kernel device time in ms, number of bracketed launches); clears the record."""
+        ms = C.c_double(0.0)
+        n = C.c_longlong(0)
+        _check(lib().lbm_kernel_timing_read(self._h, C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     def synchronize(self):
         self._stream.synchronize()

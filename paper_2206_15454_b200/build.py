@@ -21,7 +21,7 @@ NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared",
     "--fmad=true",            # FMA contraction on; no -use_fast_math (IEEE sqrt / division)
-    "-Xptxas", "-warn-spills",
+    "-Xptxas", "-warn-spills", "-diag-suppress", "177",
 ]
 
 

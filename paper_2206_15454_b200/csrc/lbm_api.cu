@@ -85,7 +85,11 @@ struct lbm_s {
     double U_ref, noise_frac;
     char variant[64];
     KParams kp;
+    bool timing;
+    std::vector<cudaEvent_t> ev; // start/stop pairs of the bracketed step-kernel launches
+    size_t ev_used;
 };
+constexpr size_t MAX_TIMED = 4096;
 
 static bool valid_top_bottom(uint32_t bc, int *bot, int *top)
 {
@@ -181,6 +185,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->ws = nullptr; h->stream = nullptr; h->bound = false; h->inited = false;
     h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
     h->init_kind = LBM_INIT_REST; h->U_ref = 0.0; h->noise_frac = 0.0;
+    h->timing = false; h->ev_used = 0;
     snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", V, h->TX, h->TY);
     *out = h;
     return LBM_OK;
@@ -418,7 +423,20 @@ int lbm_step(lbm_t *h, int n)
             p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
             p.shift = reinterpret_cast<const float *>(h->ws + h->L.shift);
         }
+        const bool timed = h->timing && h->ev_used + 2 <= 2 * MAX_TIMED;
+        if (timed) {
+            while (h->ev.size() < h->ev_used + 2) {
+                cudaEvent_t e;
+                CU_TRY(cudaEventCreate(&e));
+                h->ev.push_back(e);
+            }
+            CU_TRY(cudaEventRecord(h->ev[h->ev_used], h->stream));
+        }
         CU_TRY(launch_step(h, p, sample));
+        if (timed) {
+            CU_TRY(cudaEventRecord(h->ev[h->ev_used + 1], h->stream));
+            h->ev_used += 2;
+        }
         if (sample) {
             CU_TRY(launch_stage2(h, 0));
             h->nsamples++;
@@ -536,7 +554,36 @@ long long lbm_time(const lbm_t *h) { return h ? h->t : -1; }
 long long lbm_launch_count(const lbm_t *h) { return h ? h->launches : -1; }
 const char *lbm_variant(const lbm_t *h) { return h ? h->variant : ""; }
 
-void lbm_destroy(lbm_t *h) { delete h; }
+int lbm_set_kernel_timing(lbm_t *h, int on)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    h->timing = on != 0;
+    return LBM_OK;
+}
+
+int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_kernel_timing_read before lbm_bind");
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    double tot = 0.0;
+    for (size_t q = 0; q + 1 < h->ev_used; q += 2) {
+        float ms = 0.f;
+        CU_TRY(cudaEventElapsedTime(&ms, h->ev[q], h->ev[q + 1]));
+        tot += ms;
+    }
+    if (total_ms) *total_ms = tot;
+    if (launches) *launches = (long long)(h->ev_used / 2);
+    h->ev_used = 0;
+    return LBM_OK;
+}
+
+void lbm_destroy(lbm_t *h)
+{
+    if (!h) return;
+    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    delete h;
+}
 
 int lbm_lad_profile(int hc, int ny, double LAI, double eta_m, double *out)
 {
