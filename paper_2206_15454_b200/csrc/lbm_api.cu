@@ -257,7 +257,7 @@ int lbm_set_init(lbm_t *h, int kind, double U_ref, double noise_frac)
 template <int V>
 static cudaError_t launch_init_v(lbm_s *h, const KParams &p, int planes)
 {
-    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY), h->nchunk);
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
     if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
     else init_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
@@ -275,7 +275,7 @@ static cudaError_t launch_init(lbm_s *h, const KParams &p, int planes)
 template <int V>
 static cudaError_t launch_macros_v(lbm_s *h, const KParams &p, int planes)
 {
-    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY), h->nchunk);
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
     if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL><<<grid, block, 0, h->stream>>>(p);
     else macros_kernel<V, RD_PULL_OPP><<<grid, block, 0, h->stream>>>(p);
@@ -294,7 +294,7 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
 template <int V, bool S>
 static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
 {
-    dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY), h->nchunk);
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY * h->nchunk));
     if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S><<<grid, block, 0, h->stream>>>(p);
     else step_kernel<V, RD_PULL_OPP, WR_PUSH, S><<<grid, block, 0, h->stream>>>(p);

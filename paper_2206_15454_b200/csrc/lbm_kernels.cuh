@@ -113,20 +113,27 @@ template <int V> __device__ __forceinline__ void stv(float *p, const float (&o)[
 
 // Per-thread geometry: V cells x0..x0+V-1 of row (y, z).
 struct Ctx {
-    int x0, y, z;
+    int x0, y, z, chunk;
     int xl, xr;        // wrapped x0-1, x0+V
     int ym, yp, zm, zp; // neighbour rows (wrapped / clamped)
     bool bot_bb, top_bb, top_fs; // this row touches a wall / free-slip face
     bool edgeL, edgeR;  // lane has no x-neighbour lane on that side
 };
 
-template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0)
+// `again`: recompute from laundered thread/block indices, so that the compiler does not keep the
+// first Ctx alive across the collision (register pressure of the AA odd step).
+template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0, bool again = false)
 {
     Ctx c;
-    const int tx = threadIdx.x, ty = threadIdx.y;
+    int tx = threadIdx.x, ty = threadIdx.y, bx = blockIdx.x;
+    if (again) asm volatile("" : "+r"(tx), "+r"(ty), "+r"(bx));
     const int lane = (ty * blockDim.x + tx) & 31;
-    c.x0 = (blockIdx.y * blockDim.x + tx) * V;
-    const int row = row0 + blockIdx.x * blockDim.y + ty;
+    // 1-D grid, the x chunks of a row are consecutive blocks (they run together, so the partial
+    // sectors at the chunk seams of the shifted stores merge in L2)
+    const int rb = bx / p.nchunk;
+    c.chunk = bx - rb * p.nchunk;
+    c.x0 = (c.chunk * blockDim.x + tx) * V;
+    const int row = row0 + rb * blockDim.y + ty;
     c.z = row / p.ny;
     c.y = row - c.z * p.ny;
     c.xl = (c.x0 == 0) ? p.nx - 1 : c.x0 - 1;
@@ -292,6 +299,26 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, const 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Hardware approximations (MUFU.RCP / MUFU.SQRT, <= 1 ulp).  Used only where the error enters at
+// second order in the Mach number or multiplies the non-equilibrium part (DESIGN.md
+// "Arithmetic form"): 1/rho in the quadratic terms, the two square roots and the reciprocal of
+// the relaxation time.  Momentum is carried as j = rho u, so no result depends on
+// rho * (1/rho) == 1.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------
 // S2-S4: moments of the shifted populations, predictor velocity, forest drag, corrected
 // velocity and total force of one cell (Eqs. 5-7, 13; Alg. 1).
 // Pair sums/differences s_k = g_a + g_b, d_k = g_a - g_b over the 9 opposite pairs feed both the
@@ -299,6 +326,7 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, const 
 // ---------------------------------------------------------------------------------------------
 struct Cell {
     float drho, rho, inv_rho;
+    float jx, jy, jz;   // force-corrected momentum rho u = sum f c + F/2 (Eq. 6)
     float ux, uy, uz;   // force-corrected velocity (the sample S)
     float Fx, Fy, Fz;   // total force density F_b + F_f
     float Pxx, Pyy, Pzz, Pxy, Pyz, Pxz; // sum g_i c c  (= Pi - I/3)
@@ -329,74 +357,80 @@ __device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V]
     m.Pxz = s11 - s13;
     m.Pyz = s15 - s17;
     m.rho = 1.0f + m.drho;
-    m.inv_rho = 1.0f / m.rho;
-    // Alg. 1: local velocity with the driving force (Eq. 6; R7)
-    const float usx = (mx + 0.5f * p.Fbx) * m.inv_rho;
-    const float usy = (my + 0.5f * p.Fby) * m.inv_rho;
-    const float usz = (mz + 0.5f * p.Fbz) * m.inv_rho;
-    float Ffx = 0.f, Ffy = 0.f, Ffz = 0.f;
+    m.inv_rho = rcp_approx(m.rho);
+    // Alg. 1: local momentum with the driving force (Eq. 6; R7)
+    m.jx = mx + 0.5f * p.Fbx;
+    m.jy = my + 0.5f * p.Fby;
+    m.jz = mz + 0.5f * p.Fbz;
+    m.Fx = p.Fbx; m.Fy = p.Fby; m.Fz = p.Fbz;
     if (cda > 0.f) {
-        // Alg. 1, Eq. 13: F_f = -C_D a_f(y) |u| u, no rho factor (R4), streamwise only (R5)
-        const float mag = sqrtf(usx * usx + usy * usy + usz * usz);
-        const float coef = -cda * mag;
-        Ffx = coef * usx;
-        if (p.drag_vector) { Ffy = coef * usy; Ffz = coef * usz; }
+        // Alg. 1, Eq. 13: F_f = -C_D a_f(y) |u*| u*, no rho factor (R4), streamwise only (R5)
+        const float usx = m.jx * m.inv_rho, usy = m.jy * m.inv_rho, usz = m.jz * m.inv_rho;
+        const float coef = -cda * sqrt_approx(usx * usx + usy * usy + usz * usz);
+        const float Ffx = coef * usx;
+        // Alg. 1: correct the velocity with the forest force (explicit; R6)
+        m.jx += 0.5f * Ffx; m.Fx += Ffx;
+        if (p.drag_vector) {
+            const float Ffy = coef * usy, Ffz = coef * usz;
+            m.jy += 0.5f * Ffy; m.Fy += Ffy;
+            m.jz += 0.5f * Ffz; m.Fz += Ffz;
+        }
     }
-    // Alg. 1: correct the velocity with the forest force (explicit; R6)
-    const float hir = 0.5f * m.inv_rho;
-    m.ux = usx + hir * Ffx; m.uy = usy + hir * Ffy; m.uz = usz + hir * Ffz;
-    m.Fx = p.Fbx + Ffx; m.Fy = p.Fby + Ffy; m.Fz = p.Fbz + Ffz;
+    m.ux = m.jx * m.inv_rho; m.uy = m.jy * m.inv_rho; m.uz = m.jz * m.inv_rho;
     return m;
 }
 
 // S5-S6: Smagorinsky tau_total (Eqs. 10-12; R8, R9) and the forced BGK collision (Eqs. 1-4; R1,
-// R10) in even/odd pair form on the shifted populations:
-//   g*_i = (1-w) g_i + w (f_eq,i - w_i) + F_i,
-//   f_eq,i - w_i = w_i [ drho + rho (3 cu + 4.5 cu^2 - 1.5 uu) ],
-//   F_i = (1 - w/2) w_i [ 3 cF - 3 uF + 9 cu cF ],  w = 1/tau_total.
+// R10) in even/odd pair form on the shifted populations, momentum form (j = rho u):
+//   g*_i = (1-w) g_i + w (f_eq,i - w_i) + F_i,                     w = 1/tau_total
+//   f_eq,i - w_i = w_i [ drho + 3 c.j + 4.5 (c.u)(c.j) - 1.5 u.j ],
+//   F_i = (1 - w/2) w_i [ 3 c.F - 3 u.F + 9 (c.u)(c.F) ].
+// Per pair (i, opp i):  even part  w_i [ e0 + (c.u)(c.h) ],  h = 4.5 w j + 9 (1-w/2) F
+//                       odd part   w_i  c.k,                 k = 3 w j + 3 (1-w/2) F.
 template <int V>
 __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m)
 {
-    const float ux = m.ux, uy = m.uy, uz = m.uz, rho = m.rho;
+    const float ux = m.ux, uy = m.uy, uz = m.uz;
     const float third_drho = m.drho * (1.0f / 3.0f);
-    const float nxx = m.Pxx - third_drho - rho * ux * ux;   // Pi_neq = Pi - Pi_eq (L69)
-    const float nyy = m.Pyy - third_drho - rho * uy * uy;
-    const float nzz = m.Pzz - third_drho - rho * uz * uz;
-    const float nxy = m.Pxy - rho * ux * uy;
-    const float nyz = m.Pyz - rho * uy * uz;
-    const float nxz = m.Pxz - rho * ux * uz;
+    const float nxx = m.Pxx - third_drho - m.jx * ux;   // Pi_neq = Pi - Pi_eq (L69)
+    const float nyy = m.Pyy - third_drho - m.jy * uy;
+    const float nzz = m.Pzz - third_drho - m.jz * uz;
+    const float nxy = m.Pxy - m.jx * uy;
+    const float nyz = m.Pyz - m.jy * uz;
+    const float nxz = m.Pxz - m.jx * uz;
     const float QQ = (nxx * nxx + nyy * nyy + nzz * nzz) + 2.0f * (nxy * nxy + nyz * nyz + nxz * nxz);
-    const float Qh = sqrtf(QQ);                                                 // Eq. 11
-    const float tau = 0.5f * (p.tau0 + sqrtf(p.tau0sq + p.ksmag * Qh * m.inv_rho)); // Eq. 12
-    const float w = 1.0f / tau;
+    const float Qh = sqrt_approx(QQ);                                                      // Eq. 11
+    const float tau = 0.5f * (p.tau0 + sqrt_approx(p.tau0sq + p.ksmag * Qh * m.inv_rho)); // Eq. 12
+    const float w = rcp_approx(tau);
     const float omw = 1.0f - w;
     const float gp = 1.0f - 0.5f * w;                                           // Guo prefactor (R10)
-    const float uu = ux * ux + uy * uy + uz * uz;
+    const float uj = ux * m.jx + uy * m.jy + uz * m.jz;
     const float uF = ux * m.Fx + uy * m.Fy + uz * m.Fz;
-    // common even part: w (drho - 1.5 rho uu) - 3 gp uF
-    const float ev0 = w * (m.drho - 1.5f * rho * uu) - 3.0f * gp * uF;
-    const float a2 = 4.5f * w * rho;   // multiplies cu^2
-    const float a1 = 3.0f * w * rho;   // multiplies cu
-    const float b2 = 9.0f * gp;        // multiplies cu cF
-    const float b1 = 3.0f * gp;        // multiplies cF
-    g[0][k] = omw * g[0][k] + (1.0f / 3.0f) * ev0;
-#define LBM_PAIR(A, B, WGT, CU, CF)                                   \
-    {                                                                 \
-        const float cu = (CU), cF = (CF);                             \
-        const float ev = (WGT) * (ev0 + cu * (a2 * cu + b2 * cF));    \
-        const float od = (WGT) * (a1 * cu + b1 * cF);                 \
-        g[A][k] = omw * g[A][k] + (ev + od);                          \
-        g[B][k] = omw * g[B][k] + (ev - od);                          \
+    const float e0 = w * (m.drho - 1.5f * uj) - 3.0f * gp * uF;
+    const float a2 = 4.5f * w, b2 = 9.0f * gp, a1 = 3.0f * w, b1 = 3.0f * gp;
+    const float hx = a2 * m.jx + b2 * m.Fx, hy = a2 * m.jy + b2 * m.Fy, hz = a2 * m.jz + b2 * m.Fz;
+    const float kx = a1 * m.jx + b1 * m.Fx, ky = a1 * m.jy + b1 * m.Fy, kz = a1 * m.jz + b1 * m.Fz;
+    constexpr float W0 = 1.0f / 3.0f, W1 = 1.0f / 18.0f, W2 = 1.0f / 36.0f;
+    g[0][k] = omw * g[0][k] + W0 * e0;
+    // axis pairs: c.u = u_a, c.h = h_a, c.k = k_a
+    const float e1 = W1 * e0, e2 = W2 * e0;
+#define LBM_PAIR(A, B, EV, OD)                      \
+    {                                               \
+        const float ev = (EV), od = (OD);           \
+        g[A][k] = omw * g[A][k] + (ev + od);        \
+        g[B][k] = omw * g[B][k] + (ev - od);        \
     }
-    LBM_PAIR(1, 2, 1.0f / 18.0f, ux, m.Fx)
-    LBM_PAIR(3, 4, 1.0f / 18.0f, uy, m.Fy)
-    LBM_PAIR(5, 6, 1.0f / 18.0f, uz, m.Fz)
-    LBM_PAIR(7, 8, 1.0f / 36.0f, ux + uy, m.Fx + m.Fy)
-    LBM_PAIR(9, 10, 1.0f / 36.0f, ux - uy, m.Fx - m.Fy)
-    LBM_PAIR(11, 12, 1.0f / 36.0f, ux + uz, m.Fx + m.Fz)
-    LBM_PAIR(13, 14, 1.0f / 36.0f, ux - uz, m.Fx - m.Fz)
-    LBM_PAIR(15, 16, 1.0f / 36.0f, uy + uz, m.Fy + m.Fz)
-    LBM_PAIR(17, 18, 1.0f / 36.0f, uy - uz, m.Fy - m.Fz)
+    LBM_PAIR(1, 2, e1 + (W1 * ux) * hx, W1 * kx)
+    LBM_PAIR(3, 4, e1 + (W1 * uy) * hy, W1 * ky)
+    LBM_PAIR(5, 6, e1 + (W1 * uz) * hz, W1 * kz)
+    const float vx = W2 * ux, vy = W2 * uy, vz = W2 * uz;   // weight folded into c.u
+    const float qx = W2 * kx, qy = W2 * ky, qz = W2 * kz;   // weight folded into c.k
+    LBM_PAIR(7, 8, e2 + (vx + vy) * (hx + hy), qx + qy)
+    LBM_PAIR(9, 10, e2 + (vx - vy) * (hx - hy), qx - qy)
+    LBM_PAIR(11, 12, e2 + (vx + vz) * (hx + hz), qx + qz)
+    LBM_PAIR(13, 14, e2 + (vx - vz) * (hx - hz), qx - qz)
+    LBM_PAIR(15, 16, e2 + (vy + vz) * (hy + hz), qy + qz)
+    LBM_PAIR(17, 18, e2 + (vy - vz) * (hy - hz), qy - qz)
 #undef LBM_PAIR
 }
 
@@ -407,13 +441,27 @@ __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int 
 // across the warps of a segment) and stored, without atomics, to
 //   partial[(y*NSTAT + k) * (nz*nchunk) + z*nchunk + chunk].
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void stats_add(float (&s)[NSTAT], const Cell &m, float u0, float v0, float w0)
+__device__ __forceinline__ void stats_add(float (&s)[NSTAT], const Cell &m)
 {
-    const float a = m.ux - u0, b = m.uy - v0, c = m.uz - w0;
-    s[0] += a; s[1] += b; s[2] += c;
-    s[3] += a * a; s[4] += b * b; s[5] += c * c;
-    s[6] += a * b; s[7] += b * c; s[8] += a * c;
+    s[0] += m.ux; s[1] += m.uy; s[2] += m.uz;
+    s[3] += m.ux * m.ux; s[4] += m.uy * m.uy; s[5] += m.uz * m.uz;
+    s[6] += m.ux * m.uy; s[7] += m.uy * m.uz; s[8] += m.ux * m.uz;
     s[9] += m.drho;
+}
+
+// Re-centre a thread's raw sums over n cells about (u0, v0, w0): sum (a-a0)(b-b0) =
+// sum ab - a0 sum b - b0 sum a + n a0 b0.  Done once per thread, after the cell loop (the centre is
+// not live across the loop), so that the cross-thread reduction works on small numbers.
+__device__ __forceinline__ void stats_recentre(float (&s)[NSTAT], float n, float u0, float v0, float w0)
+{
+    const float a = s[0], b = s[1], c = s[2];
+    s[3] += u0 * (n * u0 - 2.0f * a);
+    s[4] += v0 * (n * v0 - 2.0f * b);
+    s[5] += w0 * (n * w0 - 2.0f * c);
+    s[6] += u0 * (n * v0 - b) - v0 * a;
+    s[7] += v0 * (n * w0 - c) - w0 * b;
+    s[8] += u0 * (n * w0 - c) - w0 * a;
+    s[0] = a - n * u0; s[1] = b - n * v0; s[2] = c - n * w0;
 }
 
 __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c, float (&s)[NSTAT])
@@ -423,31 +471,44 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
     const int TX = blockDim.x, tx = threadIdx.x, ty = threadIdx.y;
     const int lin = ty * TX + tx, warp = lin >> 5, lane = lin & 31;
     const long long pstride = (long long)p.nz * p.nchunk;
-    float *out = p.partial + ((long long)c.y * NSTAT) * pstride + (long long)c.z * p.nchunk + blockIdx.y;
+    float *out = p.partial + ((long long)c.y * NSTAT) * pstride + (long long)c.z * p.nchunk + c.chunk;
     if ((TX & 31) == 0) {
-        // every warp lies inside one row segment
+        // every warp lies inside one row segment: recursive-halving butterfly, 12 shuffles for
+        // the 10 sums (split 5|5, 3|3, 2|2, 1|1, then a plain exchange).  Afterwards the lanes
+        // 0, 2, 4, 8, 10 hold columns 0..4 and lanes 16, 18, 20, 24, 26 columns 5..9.
+        const bool b16 = lane & 16, b8 = lane & 8, b4 = lane & 4, b2 = lane & 2;
+        float v1[6], v2[4], v3[2];
 #pragma unroll
-        for (int k = 0; k < NSTAT; ++k) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+        for (int k = 0; k < 5; ++k) {
+            const float keep = b16 ? s[k + 5] : s[k], send = b16 ? s[k] : s[k + 5];
+            v1[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
         }
+        v1[5] = 0.f;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const float keep = b8 ? v1[k + 3] : v1[k], send = b8 ? v1[k] : v1[k + 3];
+            v2[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+        v2[3] = 0.f;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const float keep = b4 ? v2[k + 2] : v2[k], send = b4 ? v2[k] : v2[k + 2];
+            v3[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        }
+        float v4 = (b2 ? v3[1] : v3[0]) + __shfl_xor_sync(0xffffffffu, b2 ? v3[0] : v3[1], 2);
+        v4 += __shfl_xor_sync(0xffffffffu, v4, 1);
+        const int q = (b8 ? 3 : 0) + (b4 ? 2 : 0) + (b2 ? 1 : 0);
+        const bool owner = !(lane & 1) && q < 5 && !(b8 && b4) && !(b4 && b2);
+        const int col = (b16 ? 5 : 0) + q;
         const int wpr = TX >> 5;
         if (wpr == 1) {
-            if (lane < NSTAT) {
-                float v = s[0];
-#pragma unroll
-                for (int k = 1; k < NSTAT; ++k) v = (lane == k) ? s[k] : v;
-                out[(long long)lane * pstride] = v;
-            }
+            if (owner) out[(long long)col * pstride] = v4;
         } else {
-            if (lane == 0) {
-#pragma unroll
-                for (int k = 0; k < NSTAT; ++k) sred[warp][k] = s[k];
-            }
+            if (owner) sred[warp][col] = v4;
             __syncthreads();
             if (tx < NSTAT) {
                 float v = 0.f;
-                for (int q = 0; q < wpr; ++q) v += sred[ty * wpr + q][tx];
+                for (int w2 = 0; w2 < wpr; ++w2) v += sred[ty * wpr + w2][tx];
                 out[(long long)tx * pstride] = v;
             }
         }
@@ -487,23 +548,25 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
     load_all<V, RM>(p, c, g);
     const float cda = __ldg(p.cda + c.y);
     float s[NSTAT];
-    float u0 = 0.f, v0 = 0.f, w0 = 0.f;
     if constexpr (STATS) {
 #pragma unroll
         for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
-        if (p.shift) {
-            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c.y);
-            u0 = sh.x; v0 = sh.y; w0 = sh.z;
-        }
     }
 #pragma unroll
     for (int k = 0; k < V; ++k) {
         const Cell m = moments<V>(p, g, k, cda);
-        if constexpr (STATS) stats_add(s, m, u0, v0, w0);
+        if constexpr (STATS) stats_add(s, m);
         collide<V>(p, g, k, m);
     }
-    store_all<V, WM>(p, c, g);
-    if constexpr (STATS) stats_row_reduce(p, c, s);
+    const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, 0, true) : c;
+    store_all<V, WM>(p, c2, g);
+    if constexpr (STATS) {
+        if (p.shift) {
+            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c2.y);
+            stats_recentre(s, (float)V, sh.x, sh.y, sh.z);
+        }
+        stats_row_reduce(p, c2, s);
+    }
 }
 
 // Sample S_k without changing the state (R19): the front half of the step (S1-S4).  Writes
@@ -519,16 +582,11 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
     float s[NSTAT];
 #pragma unroll
     for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
-    float u0 = 0.f, v0 = 0.f, w0 = 0.f;
-    if (p.partial && p.shift) {
-        const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c.y);
-        u0 = sh.x; v0 = sh.y; w0 = sh.z;
-    }
     float r[V], ux[V], uy[V], uz[V];
 #pragma unroll
     for (int k = 0; k < V; ++k) {
         const Cell m = moments<V>(p, g, k, cda);
-        stats_add(s, m, u0, v0, w0);
+        stats_add(s, m);
         r[k] = m.rho; ux[k] = m.ux; uy[k] = m.uy; uz[k] = m.uz;
     }
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
@@ -538,7 +596,13 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
         stv<V>(p.u_out + p.Nio + off, uy);
         stv<V>(p.u_out + 2 * p.Nio + off, uz);
     }
-    if (p.partial) stats_row_reduce(p, c, s);
+    if (p.partial) {
+        if (p.shift) {
+            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c.y);
+            stats_recentre(s, (float)V, sh.x, sh.y, sh.z);
+        }
+        stats_row_reduce(p, c, s);
+    }
 }
 
 // splitmix64 output function of seed + (ctr+1)*golden.
