@@ -37,6 +37,10 @@ if ROOT not in sys.path:
 import workloads as wl  # noqa: E402
 
 BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star)
+# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch / cells, from the one
+# `ncu --set full` capture of the current kernel (profiles/r01_README.md: cfg4, both AA parities
+# 151.7 B/cell).  The bench line scales it by the cell count of the timed workload and says so.
+NCU_TRAFFIC_BYTES_PER_CELL = {"aa": 151.7}
 METRIC = "MLUPS"
 UNIT = "MLUPS (1e6 lattice-cell updates/s)"
 
@@ -60,6 +64,12 @@ class ClockSampler(threading.Thread):
         self.stop_flag = threading.Event()
         self.sm, self.reasons, self.sm_max, self.power = [], set(), None, []
         self.err = None
+        self.ready = threading.Event()
+
+    def begin(self):
+        """Start sampling and wait until NVML is up, so that short timed regions get samples."""
+        self.start()
+        self.ready.wait(5.0)
 
     def run(self):
         try:
@@ -73,6 +83,7 @@ class ClockSampler(threading.Thread):
                 getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
                 getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
             }
+            self.ready.set()
             while not self.stop_flag.is_set():
                 self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
                 try:
@@ -86,6 +97,7 @@ class ClockSampler(threading.Thread):
                 self.stop_flag.wait(0.1)
         except Exception as e:  # NVML missing: report it, do not fail the bench
             self.err = repr(e)
+            self.ready.set()
 
     def result(self):
         self.stop_flag.set()
@@ -232,7 +244,7 @@ def run_b200(args, cfg):
     sim.step(W)
     barrier()
     sampler = ClockSampler(local)
-    sampler.start()
+    sampler.begin()
     l0 = sim.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
@@ -289,6 +301,13 @@ def run_b200(args, cfg):
         mlups = world * N * K / (ms * 1e-3) / 1e6
         e2e_mlups = world * N * e2e_steps / (e2e_ms * 1e-3) / 1e6
         achieved = BYTES_PER_CELL * N / (kernel_ms * 1e-3) / 1e9
+        traffic, traffic_src = args.traffic, "command line (--traffic)"
+        if traffic is None and cfg["storage"] in NCU_TRAFFIC_BYTES_PER_CELL:
+            traffic = round(NCU_TRAFFIC_BYTES_PER_CELL[cfg["storage"]] * N)
+            traffic_src = ("ncu --set full on cfg4 (profiles/r01_README.md): "
+                           f"{NCU_TRAFFIC_BYTES_PER_CELL[cfg['storage']]} B/cell x {N} cells")
+        elif traffic is None:
+            traffic_src = None
         line = {
             "metric": METRIC, "value": round(mlups, 1), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": round(ms / K, 5), "higher_is_better": True,
@@ -298,7 +317,8 @@ def run_b200(args, cfg):
             "frac_of_nominal_8tbs": round(mlups * BYTES_PER_CELL / 1e3 / world / 8000.0, 4),
             "roofline": {"bound": "hbm", "kernel": "lbm::step_kernel (" + variant + ")",
                          "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                         "frac": round(achieved / peak, 4), "traffic": args.traffic,
+                         "frac": round(achieved / peak, 4), "traffic": traffic,
+                         "traffic_source": traffic_src,
                          "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL,
                          "kernel_ms": round(kernel_ms, 5), "launches_timed": k_n},
             "e2e": {"value": round(e2e_mlups, 1), "unit": UNIT,
