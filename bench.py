@@ -203,6 +203,23 @@ def workload_config(cfg, args, variant):
     return c
 
 
+def max_over_ranks(values, world: int, device):
+    """Element-wise MAX over the ranks of the default process group (times of independent
+    replicas: the job is as slow as its slowest rank).  world == 1: the values themselves."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_mlups(n_cells: int, steps: int, ms: float, world: int) -> float:
+    """Whole-job MLUPS of `world` replicas that each advanced n_cells x steps in `ms` (max)."""
+    return world * n_cells * steps / (ms * 1e-3) / 1e6
+
+
 # ---------------------------------------------------------------------------------------------
 # the CUDA leg
 # ---------------------------------------------------------------------------------------------
@@ -287,10 +304,7 @@ def run_b200(args, cfg):
     d2h = cfg["ny"] * (lb.NSTAT * 8 + 16) + 4
 
     # ---- max over ranks, sum of work ----
-    times = torch.tensor([ms, e2e_s * 1e3, kernel_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    ms, e2e_ms, kernel_ms = (float(v) for v in times.cpu())
+    ms, e2e_ms, kernel_ms = max_over_ranks([ms, e2e_s * 1e3, kernel_ms], world, dev)
     variant = sim.variant
     sim.close()
     del sim, rho_h, u_h
@@ -298,8 +312,8 @@ def run_b200(args, cfg):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        mlups = world * N * K / (ms * 1e-3) / 1e6
-        e2e_mlups = world * N * e2e_steps / (e2e_ms * 1e-3) / 1e6
+        mlups = aggregate_mlups(N, K, ms, world)
+        e2e_mlups = aggregate_mlups(N, e2e_steps, e2e_ms, world)
         achieved = BYTES_PER_CELL * N / (kernel_ms * 1e-3) / 1e9
         traffic, traffic_src = args.traffic, "command line (--traffic)"
         if traffic is None and cfg["storage"] in NCU_TRAFFIC_BYTES_PER_CELL:

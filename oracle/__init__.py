@@ -191,8 +191,11 @@ class Oracle:
 
     def __del__(self):
         h = getattr(self, "_h", None)
-        if h:
-            lib().orc_destroy(h)
+        if h and _lib is not None:      # at interpreter shutdown the module globals may be gone
+            try:
+                _lib.orc_destroy(h)
+            except Exception:
+                pass
             self._h = None
 
     @property
