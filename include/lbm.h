@@ -54,7 +54,9 @@ typedef enum lbm_status {
 #define LBM_TOP_WALL          (0u << 2)   /* bits 2-3: halfway bounce-back                            */
 #define LBM_TOP_FREE_SLIP     (1u << 2)   /*           specular reflection (BASELINE.json configs)    */
 #define LBM_TOP_PERIODIC      (2u << 2)   /*           periodic in y (must pair with BOTTOM_PERIODIC) */
+#define LBM_TOP_FORCED_EQ     (3u << 2)   /*           forced-equilibrium lid, the paper's ABL top (L216) */
 #define LBM_DRAG_VECTOR       (1u << 4)   /* bit 4: 0 streamwise-only drag (paper, L98/L103), 1 vector */
+#define LBM_SOLID_MASK        (1u << 5)   /* bit 5: a per-cell solid bit mask will be given (lbm_set_solid) */
 #define LBM_STORAGE_AA        (1u << 6)   /* bit 6: 0 two-lattice pull, 1 single-array AA pattern     */
 #define LBM_VEC_SHIFT         8           /* bits 8-10: cells per thread override (0 auto, 1, 2, 4)   */
 #define LBM_VEC_MASK          (7u << 8)
@@ -82,6 +84,23 @@ int lbm_workspace_bytes(int nx, int ny, int nz, uint32_t bc_flags, size_t *bytes
 int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs,
                const double *body_force, double Cd, const double *lad_profile,
                uint32_t bc_flags);
+
+/* Velocity of the forced-equilibrium top (LBM_TOP_FORCED_EQ; "the top boundary is
+ * forced to be in equilibrium with the same velocity as the free-stream flow"): every population
+ * entering through the top face is f_eq,i(rho = 1, U_top) (Eq. 3).  U_top: host, 3 doubles,
+ * copied; default 0.  May be called at any time; takes effect from the next step.
+ * LBM_EINVAL if the handle was not created with LBM_TOP_FORCED_EQ or a component is not finite. */
+int lbm_set_top_velocity(lbm_t *h, const double *U_top);
+
+/* Per-cell solid geometry (LBM_SOLID_MASK; "a bit mask" codes the cell kind,
+ * L226 turbulence-trip boxes).  solid_host: host, [nz][ny][nx] bytes,
+ * non-zero = solid; NULL = no solid cell.  The library packs it to 1 bit per cell (one 32-bit word
+ * per 32 x cells, 0.125 B/cell) in the workspace.  A link between a fluid and a solid cell is a
+ * halfway bounce-back link; solid cells keep the rest state, report rho = 1, u = 0 and are left out
+ * of the plane sums (the divisor of the averages stays nx*nz).  Call after lbm_bind; the state
+ * must be (re-)initialised afterwards (lbm_init / lbm_set_macros*), LBM_ESTATE from lbm_step
+ * otherwise.  Needs nx % 32 == 0 (checked at lbm_create). */
+int lbm_set_solid(lbm_t *h, const uint8_t *solid_host);
 
 /* Attach the caller-owned device workspace and stream; uploads the per-row tables.
  * Errors: LBM_ENOMEM (bytes < lbm_workspace_bytes or pointer not 256-B aligned), LBM_ECUDA. */
@@ -160,6 +179,24 @@ const char *lbm_last_error(void);
  * a_j = LAI * s(eta_j) / sum_k s(eta_k) for j < h, 0 above, eta_j = (j+1/2)/h,
  * s(eta) = r^n exp[n(1-r)], r = (1-eta_m)/(1-eta), n = 6 (eta < eta_m) or 1/2. */
 int lbm_lad_profile(int h, int ny, double LAI, double eta_m, double *out_host);
+
+/* Host helpers (no CUDA) for the paper's normalised outputs, applied to
+ * the [ny][LBM_NSTAT] table of lbm_stats_read.
+ *   lbm_wall_friction_velocity   Eq. 16 (L179) inverted: u_tau = sqrt(F H / rho), F the streamwise
+ *                                force density, H the channel half height (full height of a
+ *                                half channel), all in lattice units.
+ *   lbm_forest_friction_velocity L210: u_* = [<u'v'>^2 + <v'w'>^2]^(1/4) at y/h = 2; y = 2h is the
+ *                                face between rows 2h-1 and 2h, so the two rows are averaged.
+ *                                LBM_EINVAL unless 1 <= h and 2h < ny.
+ *   lbm_stats_normalise          out[j][0..2] = <u_a>/u_ref (L200 "<u+> = <u>/u_tau");
+ *                                out[j][3..5] = sqrt(max(<a'a'>, 0))/u_ref (the RMS components);
+ *                                out[j][6..8] = <a'b'>/u_ref^2; out[j][9] = <rho>.  out may alias
+ *                                stats.  LBM_EINVAL if u_ref <= 0.
+ *   lbm_wall_units               y+_j = (j + 1/2) u_tau / nu for the ny cell centres. */
+int lbm_wall_friction_velocity(double F, double H, double rho, double *u_tau);
+int lbm_forest_friction_velocity(const double *stats_host, int ny, int h, double *u_star);
+int lbm_stats_normalise(const double *stats_host, int ny, double u_ref, double *out_host);
+int lbm_wall_units(int ny, double u_tau, double nu, double *yplus_host);
 
 /* Counter-based uniform generator of the input recipe: splitmix64 output function of
  * seed + (ctr+1)*0x9E3779B97F4A7C15; rand01 = top 53 bits * 2^-53. */

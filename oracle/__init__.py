@@ -155,8 +155,9 @@ def lad_from_spec(forest, ny: int):
     raise ValueError(forest)
 
 
-def bc_flags(bottom: str, top: str, drag_vector: bool = False) -> int:
-    return _BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0)
+def bc_flags(bottom: str, top: str, drag_vector: bool = False, solid: bool = False) -> int:
+    return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0)
+            | (SOLID_MASK if solid else 0))
 
 
 # ---- simulation handle ----------------------------------------------------------------------
@@ -180,9 +181,12 @@ class Oracle:
     def from_config(cls, cfg: dict) -> "Oracle":
         o = cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
                 lad_from_spec(cfg["forest"], cfg["ny"]),
-                bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False)))
+                bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False),
+                         cfg.get("solid") is not None))
         if cfg.get("U_top") is not None:
             o.set_top_velocity(cfg["U_top"])
+        if cfg.get("solid") is not None:
+            o.set_solid(cfg["solid"])
         return o
 
     def init_from_config(self, cfg: dict):

@@ -15,8 +15,9 @@ from . import build as _build
 
 # bc_flags (mirrors include/lbm.h)
 BOTTOM_WALL, BOTTOM_PERIODIC = 0, 1
-TOP_WALL, TOP_FREE_SLIP, TOP_PERIODIC = 0 << 2, 1 << 2, 2 << 2
+TOP_WALL, TOP_FREE_SLIP, TOP_PERIODIC, TOP_FORCED_EQ = 0 << 2, 1 << 2, 2 << 2, 3 << 2
 DRAG_VECTOR = 1 << 4
+SOLID_MASK = 1 << 5
 STORAGE_AA = 1 << 6
 VEC_SHIFT = 8
 NSTAT = 10
@@ -26,7 +27,8 @@ INIT_POWER_LAW, INIT_PARABOLA, INIT_REST = 0, 1, 2
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ESTATE, LBM_ECUDA, LBM_EDIVERGED = 0, -1, -2, -3, -4, -5
 
 _BOTTOM = {"bounce_back": BOTTOM_WALL, "periodic": BOTTOM_PERIODIC}
-_TOP = {"bounce_back": TOP_WALL, "free_slip": TOP_FREE_SLIP, "periodic": TOP_PERIODIC}
+_TOP = {"bounce_back": TOP_WALL, "free_slip": TOP_FREE_SLIP, "periodic": TOP_PERIODIC,
+        "forced_equilibrium": TOP_FORCED_EQ}
 
 # every symbol include/lbm.h declares
 SYMBOLS = [
@@ -35,6 +37,8 @@ SYMBOLS = [
     "lbm_stats_accumulate", "lbm_stats_read", "lbm_stats_reset", "lbm_get_state", "lbm_time",
     "lbm_launch_count", "lbm_set_launch_shape", "lbm_variant", "lbm_destroy", "lbm_last_error",
     "lbm_lad_profile", "lbm_mix64", "lbm_set_kernel_timing", "lbm_kernel_timing_read",
+    "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
+    "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units",
 ]
 
 
@@ -59,6 +63,12 @@ def lib():
                                  C.c_double, dp, C.c_uint32]
         L.lbm_bind.argtypes = [vp, vp, C.c_size_t, vp]
         L.lbm_set_init.argtypes = [vp, C.c_int, C.c_double, C.c_double]
+        L.lbm_set_top_velocity.argtypes = [vp, dp]
+        L.lbm_set_solid.argtypes = [vp, C.c_void_p]
+        L.lbm_wall_friction_velocity.argtypes = [C.c_double, C.c_double, C.c_double, dp]
+        L.lbm_forest_friction_velocity.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.lbm_stats_normalise.argtypes = [dp, C.c_int, C.c_double, dp]
+        L.lbm_wall_units.argtypes = [C.c_int, C.c_double, C.c_double, dp]
         L.lbm_init.argtypes = [vp, C.c_uint64]
         L.lbm_set_macros.argtypes = [vp, fp, fp]
         L.lbm_set_macros_host.argtypes = [vp, fp, fp]
@@ -93,9 +103,10 @@ def _check(rc: int):
         raise LbmError(rc, lib().lbm_last_error().decode())
 
 
-def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa: bool = False, vec: int = 0) -> int:
+def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa: bool = False, vec: int = 0,
+             solid: bool = False) -> int:
     return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0) | (STORAGE_AA if aa else 0)
-            | (int(vec) << VEC_SHIFT))
+            | (SOLID_MASK if solid else 0) | (int(vec) << VEC_SHIFT))
 
 
 def workspace_bytes(nx: int, ny: int, nz: int, flags: int) -> int:
@@ -108,6 +119,36 @@ def lad_profile(h: int, ny: int, LAI: float, eta_m: float = 0.7) -> np.ndarray:
     out = np.zeros(ny)
     _check(lib().lbm_lad_profile(int(h), int(ny), float(LAI), float(eta_m),
                                  out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def wall_friction_velocity(F: float, H: float, rho: float = 1.0) -> float:
+    out = C.c_double(0.0)
+    _check(lib().lbm_wall_friction_velocity(float(F), float(H), float(rho), C.byref(out)))
+    return float(out.value)
+
+
+def forest_friction_velocity(stats: np.ndarray, h: int) -> float:
+    st = np.ascontiguousarray(stats, dtype=np.float64)
+    out = C.c_double(0.0)
+    _check(lib().lbm_forest_friction_velocity(_dp(st), st.shape[0], int(h), C.byref(out)))
+    return float(out.value)
+
+
+def stats_normalise(stats: np.ndarray, u_ref: float) -> np.ndarray:
+    st = np.ascontiguousarray(stats, dtype=np.float64)
+    out = np.empty_like(st)
+    _check(lib().lbm_stats_normalise(_dp(st), st.shape[0], float(u_ref), _dp(out)))
+    return out
+
+
+def wall_units(ny: int, u_tau: float, nu: float) -> np.ndarray:
+    out = np.empty(int(ny))
+    _check(lib().lbm_wall_units(int(ny), float(u_tau), float(nu), _dp(out)))
     return out
 
 
@@ -166,11 +207,16 @@ class Lbm:
     def from_config(cls, cfg: dict, aa=None, vec: int = 0, **kw) -> "Lbm":
         if aa is None:
             aa = cfg.get("storage", "two_lattice") == "aa"
-        flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec)
+        flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec,
+                         solid=cfg.get("solid") is not None)
         s = cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
                 lad_from_spec(cfg["forest"], cfg["ny"]), flags, **kw)
         i = cfg["init"]
         s.set_init(i["kind"], i["U_ref"], i["noise_frac"])
+        if cfg.get("U_top") is not None:
+            s.set_top_velocity(cfg["U_top"])
+        if cfg.get("solid") is not None:
+            s.set_solid(cfg["solid"])
         return s
 
     def close(self):
@@ -204,6 +250,22 @@ class Lbm:
 
     def set_launch_shape(self, tx: int, ty: int):
         _check(lib().lbm_set_launch_shape(self._h, int(tx), int(ty)))
+
+    def set_solid(self, mask):
+        """mask: (nz, ny, nx) array, non-zero = solid; None clears.  Re-initialise afterwards."""
+        if mask is None:
+            _check(lib().lbm_set_solid(self._h, None))
+            return
+        m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
+        if m.shape != self.shape:
+            raise ValueError(f"solid mask must have shape {self.shape}")
+        _check(lib().lbm_set_solid(self._h, C.c_void_p(m.ctypes.data)))
+
+    def set_top_velocity(self, U):
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        if U.shape != (3,):
+            raise ValueError("U_top must have 3 components")
+        _check(lib().lbm_set_top_velocity(self._h, U.ctypes.data_as(C.POINTER(C.c_double))))
 
     def set_init(self, kind: int, U_ref: float, noise_frac: float):
         _check(lib().lbm_set_init(self._h, int(kind), float(U_ref), float(noise_frac)))

@@ -37,11 +37,11 @@ constexpr int MAX_NCHUNK = 8;
 constexpr size_t STAGING_BUDGET = (size_t)256 << 20;
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, solid, staging, total;
     int stage_planes;
 };
 
-static Layout make_layout(int nx, int ny, int nz, bool aa)
+static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
 {
     Layout L;
     const size_t N = (size_t)nx * ny * nz;
@@ -54,6 +54,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa)
     L.cda = off; off = align_up(off + (size_t)ny * 4, 256);
     L.uprof = off; off = align_up(off + (size_t)ny * 4, 256);
     L.flag = off; off += 256;
+    L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     const size_t plane = (size_t)16 * nx * ny;
     size_t planes = STAGING_BUDGET / plane;
     if (planes < 1) planes = 1;
@@ -67,11 +68,12 @@ static Layout make_layout(int nx, int ny, int nz, bool aa)
 struct lbm_s {
     int nx, ny, nz;
     long long N;
-    double nu, Cs, Fb[3], Cd;
+    double nu, Cs, Fb[3], Cd, Utop[3];
     std::vector<double> lad;
     uint32_t bc;
     int bot, top;
-    bool aa, drag_vector;
+    bool aa, drag_vector, mask;
+    std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
     int V, TX, TY, nchunk;
     Layout L;
     char *ws;
@@ -94,7 +96,7 @@ constexpr size_t MAX_TIMED = 4096;
 static bool valid_top_bottom(uint32_t bc, int *bot, int *top)
 {
     const int b = bc & 3u, t = (bc >> 2) & 3u;
-    if (b > 1 || t > 2) return false;
+    if (b > 1) return false;
     if ((b == 1) != (t == 2)) return false; // periodic-y needs both faces
     *bot = b; *top = t;
     return true;
@@ -138,7 +140,7 @@ int lbm_workspace_bytes(int nx, int ny, int nz, uint32_t bc_flags, size_t *bytes
     if (!bytes) return fail(LBM_EINVAL, "bytes is NULL");
     if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "lattice sizes must be >= 1");
     if ((double)nx * ny * nz >= 2147483648.0) return fail(LBM_EINVAL, "nx*ny*nz must be < 2^31");
-    *bytes = make_layout(nx, ny, nz, (bc_flags & LBM_STORAGE_AA) != 0).total;
+    *bytes = make_layout(nx, ny, nz, (bc_flags & LBM_STORAGE_AA) != 0, (bc_flags & LBM_SOLID_MASK) != 0).total;
     return LBM_OK;
 }
 
@@ -152,10 +154,12 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     if (!(nu > 0.0) || !std::isfinite(nu)) return fail(LBM_EINVAL, "nu must be > 0 (got %g)", nu);
     if (!(Cs >= 0.0) || !std::isfinite(Cs)) return fail(LBM_EINVAL, "Cs must be >= 0 (got %g)", Cs);
     if (!(Cd >= 0.0) || !std::isfinite(Cd)) return fail(LBM_EINVAL, "Cd must be >= 0 (got %g)", Cd);
-    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_STORAGE_AA | LBM_VEC_MASK))
+    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_SOLID_MASK | LBM_STORAGE_AA | LBM_VEC_MASK))
         return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
     int bot, top;
     if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
+    if ((bc_flags & LBM_SOLID_MASK) && nx % 32)
+        return fail(LBM_EINVAL, "LBM_SOLID_MASK needs nx %% 32 == 0 (got nx=%d)", nx);
     const int V = pick_vec(nx, bc_flags);
     if (V < 0) return fail(LBM_EINVAL, "cells-per-thread override does not divide nx=%d", nx);
     lbm_s *h = new (std::nothrow) lbm_s();
@@ -181,11 +185,14 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
         return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
     }
     h->nchunk = (nx / V) / h->TX;
-    h->L = make_layout(nx, ny, nz, h->aa);
+    h->mask = (bc_flags & LBM_SOLID_MASK) != 0;
+    h->nfluid.assign(ny, (double)nx * nz);
+    h->L = make_layout(nx, ny, nz, h->aa, h->mask);
     h->ws = nullptr; h->stream = nullptr; h->bound = false; h->inited = false;
     h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
     h->init_kind = LBM_INIT_REST; h->U_ref = 0.0; h->noise_frac = 0.0;
     h->timing = false; h->ev_used = 0;
+    h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
     snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", V, h->TX, h->TY);
     *out = h;
     return LBM_OK;
@@ -218,6 +225,19 @@ static void fill_params(lbm_s *h)
     p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
     p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
+    {
+        // lid populations f_eq,i(1, U_top) - w_i (Eq. 3) of the five directions with c_y = -1
+        static const int li[5] = {4, 8, 9, 16, 18};
+        const double *U = h->Utop, uu = U[0] * U[0] + U[1] * U[1] + U[2] * U[2];
+        for (int q = 0; q < 5; ++q) {
+            const int i = li[q];
+            const double cu = Lat::cx[i] * U[0] + Lat::cy[i] * U[1] + Lat::cz[i] * U[2];
+            const double w = (i < 7) ? 1.0 / 18.0 : 1.0 / 36.0;
+            p.lid[q] = (float)(w * (3.0 * cu + 4.5 * cu * cu - 1.5 * uu));
+        }
+    }
+    p.solid = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid) : nullptr;
+    p.nxw = (h->nx + 31) / 32;
     p.partial = nullptr; p.shift = nullptr;
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
     p.z0 = 0; p.z1 = h->nz; p.zoff = 0; p.Nio = h->N;
@@ -238,8 +258,46 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
+    if (h->mask)
+        CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream)); // cda is a local vector
     h->bound = true; h->inited = false;
+    return LBM_OK;
+}
+
+int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->mask) return fail(LBM_EINVAL, "handle was not created with LBM_SOLID_MASK");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_solid before lbm_bind");
+    const int nxw = (h->nx + 31) / 32;
+    const size_t words = (size_t)nxw * h->ny * h->nz;
+    std::vector<uint32_t> bits;
+    try { bits.assign(words, 0u); } catch (...) { return fail(LBM_ENOMEM, "host allocation failed"); }
+    h->nfluid.assign(h->ny, (double)h->nx * h->nz);
+    if (solid_host)
+        for (int z = 0; z < h->nz; ++z)
+            for (int y = 0; y < h->ny; ++y) {
+                const uint8_t *row = solid_host + ((size_t)z * h->ny + y) * h->nx;
+                uint32_t *out = bits.data() + ((size_t)z * h->ny + y) * nxw;
+                for (int x = 0; x < h->nx; ++x)
+                    if (row[x]) { out[x >> 5] |= 1u << (x & 31); h->nfluid[y] -= 1.0; }
+            }
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    h->inited = false;   // the populations must be rebuilt around the new geometry
+    return LBM_OK;
+}
+
+int lbm_set_top_velocity(lbm_t *h, const double *U_top)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!U_top) return fail(LBM_EINVAL, "U_top is NULL");
+    if (h->top != BC_TOP_LID) return fail(LBM_EINVAL, "handle was not created with LBM_TOP_FORCED_EQ");
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(U_top[a])) return fail(LBM_EINVAL, "U_top[%d] is not finite", a);
+    for (int a = 0; a < 3; ++a) h->Utop[a] = U_top[a];
+    if (h->bound) fill_params(h);
     return LBM_OK;
 }
 
@@ -258,7 +316,10 @@ template <int V>
 static cudaError_t launch_init_v(lbm_s *h, const KParams &p, int planes)
 {
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
-    if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
+    if (h->mask) {
+        if (h->aa) init_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p);
+        else init_kernel<V, WR_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
+    } else if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
     else init_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
     return cudaGetLastError();
@@ -276,7 +337,11 @@ template <int V>
 static cudaError_t launch_macros_v(lbm_s *h, const KParams &p, int planes)
 {
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
-    if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
+    if (h->mask) {
+        if (!h->aa) macros_kernel<V, RD_PULL, true><<<grid, block, 0, h->stream>>>(p);
+        else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
+        else macros_kernel<V, RD_PULL_OPP, true><<<grid, block, 0, h->stream>>>(p);
+    } else if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL><<<grid, block, 0, h->stream>>>(p);
     else macros_kernel<V, RD_PULL_OPP><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
@@ -295,7 +360,11 @@ template <int V, bool S>
 static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
 {
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY * h->nchunk));
-    if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
+    if (h->mask) {
+        if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S, true><<<grid, block, 0, h->stream>>>(p);
+        else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S, true><<<grid, block, 0, h->stream>>>(p);
+        else step_kernel<V, RD_PULL_OPP, WR_PUSH, S, true><<<grid, block, 0, h->stream>>>(p);
+    } else if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S><<<grid, block, 0, h->stream>>>(p);
     else step_kernel<V, RD_PULL_OPP, WR_PUSH, S><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
@@ -327,8 +396,9 @@ static int stats_reset_impl(lbm_s *h)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
     h->nsamples = 0; h->stats_phase = 0;
-    if (h->inited) {
-        // centre the accumulation on the current plane means (numerical shift only)
+    if (h->inited && !h->mask) {
+        // centre the accumulation on the current plane means (numerical shift only; not with a
+        // solid mask, where the number of contributing cells differs from thread to thread)
         KParams p = h->kp;
         p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
         p.shift = nullptr;
@@ -421,7 +491,7 @@ int lbm_step(lbm_t *h, int n)
         if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
         if (sample) {
             p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
-            p.shift = reinterpret_cast<const float *>(h->ws + h->L.shift);
+            p.shift = h->mask ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
         }
         const bool timed = h->timing && h->ev_used + 2 <= 2 * MAX_TIMED;
         if (timed) {
@@ -544,7 +614,7 @@ int lbm_stats_read(lbm_t *h, double *out, long long *nsamples)
         r[0] = mu + shift[y * 4 + 0]; r[1] = mv + shift[y * 4 + 1]; r[2] = mw + shift[y * 4 + 2];
         r[3] = a[3] / cnt - mu * mu; r[4] = a[4] / cnt - mv * mv; r[5] = a[5] / cnt - mw * mw;
         r[6] = a[6] / cnt - mu * mv; r[7] = a[7] / cnt - mv * mw; r[8] = a[8] / cnt - mu * mw;
-        r[9] = 1.0 + a[9] / cnt;
+        r[9] = (a[9] + (double)h->nsamples * h->nfluid[y]) / cnt;   // sum of rho = sum(rho-1) + fluid cells
     }
     if (flag) return fail(LBM_EDIVERGED, "non-finite plane sum of rho seen by the statistics reduction");
     return LBM_OK;
@@ -602,6 +672,46 @@ int lbm_lad_profile(int hc, int ny, double LAI, double eta_m, double *out)
         out[j] = s; sum += s;
     }
     for (int j = 0; j < ny; ++j) out[j] = (sum > 0.0) ? out[j] * (LAI / sum) : 0.0;
+    return LBM_OK;
+}
+
+int lbm_wall_friction_velocity(double F, double H, double rho, double *u_tau)
+{
+    if (!u_tau) return fail(LBM_EINVAL, "u_tau is NULL");
+    if (!(F >= 0.0) || !(H > 0.0) || !(rho > 0.0)) return fail(LBM_EINVAL, "need F >= 0, H > 0, rho > 0");
+    *u_tau = std::sqrt(F * H / rho);   // Eq. 16 (L179): F = rho u_tau^2 / H
+    return LBM_OK;
+}
+
+int lbm_forest_friction_velocity(const double *stats, int ny, int hc, double *u_star)
+{
+    if (!stats || !u_star) return fail(LBM_EINVAL, "NULL argument");
+    if (hc < 1 || 2 * hc >= ny) return fail(LBM_EINVAL, "need 1 <= h and 2h < ny (h=%d, ny=%d)", hc, ny);
+    const double *lo = stats + (size_t)(2 * hc - 1) * LBM_NSTAT, *hi = stats + (size_t)(2 * hc) * LBM_NSTAT;
+    const double uv = 0.5 * (lo[6] + hi[6]), vw = 0.5 * (lo[7] + hi[7]);
+    *u_star = std::sqrt(std::sqrt(uv * uv + vw * vw));   // L210
+    return LBM_OK;
+}
+
+int lbm_stats_normalise(const double *stats, int ny, double u_ref, double *out)
+{
+    if (!stats || !out || ny < 1) return fail(LBM_EINVAL, "bad arguments");
+    if (!(u_ref > 0.0)) return fail(LBM_EINVAL, "u_ref must be > 0");
+    for (int j = 0; j < ny; ++j) {
+        const double *a = stats + (size_t)j * LBM_NSTAT;
+        double *r = out + (size_t)j * LBM_NSTAT;
+        for (int k = 0; k < 3; ++k) r[k] = a[k] / u_ref;
+        for (int k = 3; k < 6; ++k) r[k] = std::sqrt(a[k] > 0.0 ? a[k] : 0.0) / u_ref;
+        for (int k = 6; k < 9; ++k) r[k] = a[k] / (u_ref * u_ref);
+        r[9] = a[9];
+    }
+    return LBM_OK;
+}
+
+int lbm_wall_units(int ny, double u_tau, double nu, double *yplus)
+{
+    if (!yplus || ny < 1 || !(nu > 0.0) || !(u_tau >= 0.0)) return fail(LBM_EINVAL, "bad arguments");
+    for (int j = 0; j < ny; ++j) yplus[j] = (j + 0.5) * u_tau / nu;
     return LBM_OK;
 }
 

@@ -53,7 +53,7 @@ enum WriteMode { WR_LOCAL = 0,     // B[i][x]                      (two-lattice)
 };
 
 enum { BC_BOT_WALL = 0, BC_BOT_PERIODIC = 1 };
-enum { BC_TOP_WALL = 0, BC_TOP_SLIP = 1, BC_TOP_PERIODIC = 2 };
+enum { BC_TOP_WALL = 0, BC_TOP_SLIP = 1, BC_TOP_PERIODIC = 2, BC_TOP_LID = 3 };
 
 struct KParams {
     float *src;          // population array read  [19][N]
@@ -66,6 +66,9 @@ struct KParams {
     float Fbx, Fby, Fbz;        // body force density F_b
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
     int bot, top, drag_vector;
+    const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
+    int nxw;                    // words per x row (nx / 32)
+    float lid[5];               // forced-equilibrium lid: f_eq,i(1, U_top) - w_i for i = 4, 8, 9, 16, 18
     // statistics
     float *partial;             // [ny][NSTAT][nz*nchunk]
     const float *shift;         // [ny][4] accumulation centre (u0, v0, w0, -), may be NULL
@@ -116,7 +119,7 @@ struct Ctx {
     int x0, y, z, chunk;
     int xl, xr;        // wrapped x0-1, x0+V
     int ym, yp, zm, zp; // neighbour rows (wrapped / clamped)
-    bool bot_bb, top_bb, top_fs; // this row touches a wall / free-slip face
+    bool bot_bb, top_bb, top_fs, top_lid; // this row touches a wall / free-slip / lid face
     bool edgeL, edgeR;  // lane has no x-neighbour lane on that side
 };
 
@@ -144,7 +147,9 @@ template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int r
     c.ym = isbot ? (p.bot == BC_BOT_PERIODIC ? p.ny - 1 : c.y) : c.y - 1;
     c.yp = istop ? (p.top == BC_TOP_PERIODIC ? 0 : c.y) : c.y + 1;
     c.bot_bb = isbot && p.bot == BC_BOT_WALL;
-    c.top_bb = istop && p.top == BC_TOP_WALL;
+    // the lid face addresses like a wall (own cell, opposite slot); loads then take the lid value
+    c.top_lid = istop && p.top == BC_TOP_LID;
+    c.top_bb = istop && (p.top == BC_TOP_WALL || p.top == BC_TOP_LID);
     c.top_fs = istop && p.top == BC_TOP_SLIP;
     c.edgeL = (lane == 0) || (tx == 0);
     c.edgeR = (lane == 31) || (tx == (int)blockDim.x - 1);
@@ -217,8 +222,9 @@ __device__ __forceinline__ void load_dir(const KParams &p, const Ctx &c, float (
 //                             mir(I) at (x + c_x, y, z + c_z) - the places where the next even
 //                             step expects its incoming populations.
 // ---------------------------------------------------------------------------------------------
+// `act` = false: the lane takes part in the shuffles but stores nothing (solid-mask slow path).
 template <int V, int WM, int I>
-__device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const float (&r)[V])
+__device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const float (&r)[V], bool act = true)
 {
     constexpr int cx = Lat::cx[I], cy = Lat::cy[I], cz = Lat::cz[I];
     if constexpr (WM != WR_PUSH) {
@@ -237,14 +243,15 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
         const int zrow = bb ? c.z : zsel;
         float *rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
         if constexpr (cx == 0) {
-            stv<V>(rowp + c.x0, r);
+            if (act) stv<V>(rowp + c.x0, r);
         } else if constexpr (V == 1) {
             const int xs = bb ? c.x0 : (cx == 1 ? c.xr : c.xl);
-            rowp[xs] = r[0];
+            if (act) rowp[xs] = r[0];
         } else {
             if constexpr (cx == 1) {           // values land on x0+1 .. x0+V
                 const float l = __shfl_up_sync(0xffffffffu, r[V - 1], 1);
-                if (bb) {
+                if (!act) {
+                } else if (bb) {
                     stv<V>(rowp + c.x0, r);
                 } else {
                     if (!c.edgeL) {
@@ -261,7 +268,8 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
                 }
             } else {                            // values land on x0-1 .. x0+V-2
                 const float rr = __shfl_down_sync(0xffffffffu, r[0], 1);
-                if (bb) {
+                if (!act) {
+                } else if (bb) {
                     stv<V>(rowp + c.x0, r);
                 } else {
                     if (!c.edgeR) {
@@ -281,21 +289,158 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
     }
 }
 
-template <int V, int RM>
-__device__ __forceinline__ void load_all(const KParams &p, const Ctx &c, float (&g)[Q][V])
+// Forced-equilibrium top ("the top boundary is forced to be in equilibrium with the
+// same velocity as the free-stream flow"): the populations that enter
+// through the top face are f_eq,i(1, U_top), whatever the storage holds there.
+__host__ __device__ constexpr int lid_index(int i)
+{
+    return i == 4 ? 0 : i == 8 ? 1 : i == 9 ? 2 : i == 16 ? 3 : i == 18 ? 4 : -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-cell solid mask (PAPER.md:L129-135 bit-coded geometry, L226 trip boxes; SURVEY.md §8(f)
+// NEXT #2).  One bit per cell, word = 32 consecutive x cells of a row.  A link whose other end is
+// a solid cell is a halfway bounce-back link, exactly like a wall face; solid cells themselves
+// keep the rest state (g = 0) and are never updated.
+//
+// A thread gathers, for each of the 9 (y, z) rows its links touch, the V+2 bits of the cells
+// x0-1 .. x0+V into 6-bit fields packed in one 64-bit word: field (a, b), a in {ym, y, yp},
+// b in {zm, z, zp}, at bit 6*(3a + b); bit 0 = cell x0-1, bit k+1 = cell x0+k.
+// ---------------------------------------------------------------------------------------------
+template <int V>
+__device__ __forceinline__ unsigned solid_field(const KParams &p, const Ctx &c, int yrow, int zrow)
+{
+    const unsigned *row = p.solid + (long long)(yrow + p.ny * zrow) * p.nxw;
+    const int w = c.x0 >> 5, b = c.x0 & 31;
+    const unsigned m = __ldg(row + w);
+    unsigned f = ((m >> b) & ((1u << V) - 1u)) << 1;
+    if (b > 0) f |= (m >> (b - 1)) & 1u;
+    else f |= __ldg(row + (w == 0 ? p.nxw - 1 : w - 1)) >> 31;
+    if (b + V < 32) f |= ((m >> (b + V)) & 1u) << (V + 1);
+    else f |= (__ldg(row + (w + 1 == p.nxw ? 0 : w + 1)) & 1u) << (V + 1);
+    return f;
+}
+
+template <int V>
+__device__ __forceinline__ unsigned long long solid_gather(const KParams &p, const Ctx &c)
+{
+    const int ys[3] = {c.ym, c.y, c.yp}, zs[3] = {c.zm, c.z, c.zp};
+    unsigned long long S = 0ull;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+            S |= (unsigned long long)solid_field<V>(p, c, ys[a], zs[b]) << (6 * (3 * a + b));
+    return S;
+}
+__device__ __forceinline__ unsigned solid_pick(unsigned long long S, int a, int b)
+{
+    return (unsigned)(S >> (6 * (3 * a + b))) & 63u;
+}
+// own cells of the thread: bit k = cell x0+k is solid
+template <int V> __device__ __forceinline__ unsigned solid_self(unsigned long long S)
+{
+    return (solid_pick(S, 1, 1) >> 1) & ((1u << V) - 1u);
+}
+
+template <int V, int RM, bool MASK>
+__device__ __forceinline__ void load_all(const KParams &p, const Ctx &c, float (&g)[Q][V],
+                                         unsigned long long S = 0ull)
 {
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
+        constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
         load_dir<V, RM, i>(p, c, g[i]);
+        if constexpr (MASK && RM != RD_LOCAL && i != 0) {
+            // source cells of this link: (x0+k - c_x) in the row load_dir used
+            bool bb = false, fs = false;
+            if constexpr (cy == 1) bb = c.bot_bb;
+            if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
+            const int a = (bb || fs) ? 1 : 1 - cy, b = bb ? 1 : 1 - cz;
+            const unsigned bits = bb ? 0u : (solid_pick(S, a, b) >> (1 - cx)) & ((1u << V) - 1u);
+            if (bits) {                      // bounce back off the solid neighbour (own cell)
+                constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[i] : i;
+                float own[V];
+                ldv<V>(p.src + (long long)S_BB * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), own);
+#pragma unroll
+                for (int k = 0; k < V; ++k)
+                    if ((bits >> k) & 1u) g[i][k] = own[k];
+            }
+        }
+        if constexpr (cy == -1) {
+            if (c.top_lid) {
+#pragma unroll
+                for (int k = 0; k < V; ++k) g[i][k] = p.lid[lid_index(i)];
+            }
+        }
     });
 }
-template <int V, int WM>
-__device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, const float (&g)[Q][V])
+
+template <int V, int WM, bool MASK>
+__device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float (&g)[Q][V],
+                                          unsigned long long S = 0ull)
 {
-    static_for<0, Q>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        store_dir<V, WM, i>(p, c, g[i]);
-    });
+    if constexpr (!MASK) {
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            store_dir<V, WM, i>(p, c, g[i]);
+        });
+    } else if constexpr (WM != WR_PUSH) {
+        const unsigned self = solid_self<V>(S);
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+#pragma unroll
+            for (int k = 0; k < V; ++k)
+                if ((self >> k) & 1u) g[i][k] = 0.f;       // solid cells keep the rest state
+            store_dir<V, WM, i>(p, c, g[i]);
+        });
+    } else {
+        const unsigned selff = solid_pick(S, 1, 1), self = solid_self<V>(S);
+        const long long own = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
+            bool bb = false, fs = false;
+            if constexpr (cy == -1) bb = c.bot_bb;
+            if constexpr (cy == 1) { bb = c.top_bb; fs = c.top_fs; }
+            const int a = (bb || fs) ? 1 : 1 + cy, b = bb ? 1 : 1 + cz;
+            const unsigned destf = bb ? 0u : solid_pick(S, a, b);
+            // fast (vector) path only where neither the own cells, their x neighbours nor the
+            // destination cells are solid
+            const bool fast = (i == 0) ? (self == 0u) : ((selff | destf) == 0u);
+            store_dir<V, WM, i>(p, c, g[i], fast);
+            // the element a vector-path x neighbour expects THIS lane to store for it
+            float nb = 0.f;
+            if constexpr (V > 1 && cx == 1) nb = __shfl_up_sync(0xffffffffu, g[i][V - 1], 1);
+            if constexpr (V > 1 && cx == -1) nb = __shfl_down_sync(0xffffffffu, g[i][0], 1);
+            if (!fast) {
+                const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.yp : c.ym);
+                const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zp : c.zm);
+                constexpr int S_FS = Lat::mir[i], S_OPP = Lat::opp[i];
+                const int slot = fs ? S_FS : i;
+                const int yrow = fs ? c.y : ysel;
+                float *rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zsel) * p.nx;
+                float *ownp = p.dst + (long long)S_OPP * p.N + own;
+#pragma unroll
+                for (int k = 0; k < V; ++k) {
+                    if ((self >> k) & 1u) continue;                       // solid source: nothing leaves it
+                    if (bb || ((destf >> (k + cx + 1)) & 1u)) ownp[k] = g[i][k];   // bounced link
+                    else {
+                        int xd = c.x0 + k + cx;
+                        xd = (xd < 0) ? p.nx - 1 : (xd >= p.nx ? 0 : xd);
+                        rowp[xd] = g[i][k];
+                    }
+                }
+                if constexpr (V > 1 && cx == 1) {
+                    if (!bb && !c.edgeL && !(selff & 1u) && !((destf >> 1) & 1u)) rowp[c.x0] = nb;
+                }
+                if constexpr (V > 1 && cx == -1) {
+                    if (!bb && !c.edgeR && !((selff >> (V + 1)) & 1u) && !((destf >> V) & 1u))
+                        rowp[c.x0 + V - 1] = nb;
+                }
+            }
+        });
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -540,12 +685,14 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
 // ---------------------------------------------------------------------------------------------
 template <int V> struct Occ { static constexpr int minb = (V == 4) ? 2 : (V == 2 ? 3 : 4); };
 
-template <int V, int RM, int WM, bool STATS>
+template <int V, int RM, int WM, bool STATS, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, 0);
+    unsigned long long S = 0ull;
+    if constexpr (MASK) S = solid_gather<V>(p, c);
     float g[Q][V];
-    load_all<V, RM>(p, c, g);
+    load_all<V, RM, MASK>(p, c, g, S);
     const float cda = __ldg(p.cda + c.y);
     float s[NSTAT];
     if constexpr (STATS) {
@@ -555,11 +702,15 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
 #pragma unroll
     for (int k = 0; k < V; ++k) {
         const Cell m = moments<V>(p, g, k, cda);
-        if constexpr (STATS) stats_add(s, m);
+        if constexpr (STATS) {
+            // solid cells are left out of the plane sums (the divisor stays nx*nz, as in the
+            // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
+            if (!MASK || !((solid_self<V>(S) >> k) & 1u)) stats_add(s, m);
+        }
         collide<V>(p, g, k, m);
     }
     const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, 0, true) : c;
-    store_all<V, WM>(p, c2, g);
+    store_all<V, WM, MASK>(p, c2, g, S);
     if constexpr (STATS) {
         if (p.shift) {
             const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c2.y);
@@ -572,12 +723,14 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
 // Sample S_k without changing the state (R19): the front half of the step (S1-S4).  Writes
 // rho/u when the pointers are given and the stage-1 sums when p.partial is given.
 // Covers rows [z0*ny, z1*ny).
-template <int V, int RM>
+template <int V, int RM, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
+    unsigned long long S = 0ull;
+    if constexpr (MASK) S = solid_gather<V>(p, c);
     float g[Q][V];
-    load_all<V, RM>(p, c, g);
+    load_all<V, RM, MASK>(p, c, g, S);
     const float cda = __ldg(p.cda + c.y);
     float s[NSTAT];
 #pragma unroll
@@ -586,8 +739,10 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
 #pragma unroll
     for (int k = 0; k < V; ++k) {
         const Cell m = moments<V>(p, g, k, cda);
-        stats_add(s, m);
-        r[k] = m.rho; ux[k] = m.ux; uy[k] = m.uy; uz[k] = m.uz;
+        const bool solid = MASK && ((solid_self<V>(S) >> k) & 1u);
+        if (!solid) stats_add(s, m);
+        r[k] = solid ? 1.0f : m.rho;             // solid cells report the rest state
+        ux[k] = solid ? 0.f : m.ux; uy[k] = solid ? 0.f : m.uy; uz[k] = solid ? 0.f : m.uz;
     }
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
     if (p.rho_out) stv<V>(p.rho_out + off, r);
@@ -617,10 +772,12 @@ __host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long 
 // State 0 (R17): g_i = f_eq,i(rho, u) - w_i with (rho, u) from the caller's fields or from the
 // synthetic recipe (R16), written in the representation the storage scheme wants
 // (WR_LOCAL: two-lattice; WR_PUSH: AA at even t).  Covers rows [z0*ny, z1*ny).
-template <int V, int WM>
+template <int V, int WM, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
+    unsigned long long S = 0ull;
+    if constexpr (MASK) S = solid_gather<V>(p, c);
     float g[Q][V];
     const long long cell0 = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
@@ -641,6 +798,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const K
             uy = (float)(p.noise_amp * (2.0 * r1 - 1.0));
             uz = (float)(p.noise_amp * (2.0 * r2 - 1.0));
         }
+        if (MASK && ((solid_self<V>(S) >> k) & 1u)) { rho = 1.0f; ux = uy = uz = 0.f; }  // rest state
         const float drho = rho - 1.0f;
         const float uu = ux * ux + uy * uy + uz * uz;
         const float e0 = drho - 1.5f * rho * uu;
@@ -653,14 +811,21 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const K
             g[i][k] = wgt * (e0 + rho * cu * (3.0f + 4.5f * cu));
         });
     }
-    store_all<V, WM>(p, c, g);
+    store_all<V, WM, MASK>(p, c, g, S);
+}
+
+__device__ __forceinline__ bool solid_at(const KParams &p, int x, int y, int z)
+{
+    if (!p.solid) return false;
+    return (p.solid[(long long)(y + p.ny * z) * p.nxw + (x >> 5)] >> (x & 31)) & 1u;
 }
 
 // Plain "state k" (post-collision, un-streamed) populations out of whatever representation the
 // storage holds: out[i][cell] = g*_i(cell).  One cell per thread (checkpoint / tests only).
 //   two-lattice          : src[i][x]
 //   AA, t odd            : src[opp i][x]
-//   AA, t even (PUSH)    : src[i][x + c_i] with the wall / free-slip redirections of store_dir
+//   AA, t even (PUSH)    : src[i][x + c_i] with the wall / free-slip / solid redirections of
+//                          store_all; solid cells report the rest state (0)
 template <int MODE>
 __global__ void state_kernel(const KParams p, float *out)
 {
@@ -669,6 +834,7 @@ __global__ void state_kernel(const KParams p, float *out)
     const int x = (int)(cell % p.nx);
     const long long row = cell / p.nx;
     const int y = (int)(row % p.ny), z = (int)(row / p.ny);
+    const bool self_solid = solid_at(p, x, y, z);
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
@@ -688,9 +854,10 @@ __global__ void state_kernel(const KParams p, float *out)
                 else if (p.top == BC_TOP_SLIP) { slot = S_MIR; yd = y; }
                 else { slot = S_OPP; xd = x; yd = y; zd = z; }
             }
+            if (solid_at(p, xd, yd, zd)) { slot = S_OPP; xd = x; yd = y; zd = z; }
             v = p.src[(long long)slot * p.N + ((long long)(yd + p.ny * zd) * p.nx + xd)];
         }
-        out[(long long)i * p.N + cell] = v;
+        out[(long long)i * p.N + cell] = self_solid ? 0.f : v;
     });
 }
 

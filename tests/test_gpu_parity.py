@@ -294,6 +294,103 @@ def test_full_size_sampled_boxes(orc, gpu, name, aa):
         torch.cuda.empty_cache()
 
 
+# ---------------------------------------------------------------------------------------------
+# forced-equilibrium lid (NEXT #1)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (34, 2), (33, 1)])
+def test_forced_equilibrium_lid_parity(orc, gpu, aa, nx, vec):
+    cfg = wl.small(nx=nx, ny=10, nz=6, top=wl.FORCED_EQ)
+    cfg["U_top"] = (0.06, 0.0, 0.01)
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    assert _state_err(o, g, w) <= 5e-8
+    for n in (1, 2, 5, 12):                       # odd and even numbers of steps (AA parities)
+        o.step(n)
+        g.step(n)
+        er, eu = _macro_err(o, g)
+        assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+    # the lid drives the top row: its mean velocity has moved towards U_top
+    _, ug = g.get_macros()
+    assert float(ug[0, :, -1, :].mean()) > float(ug[0, :, -3, :].mean())
+
+
+def test_couette_closed_form_on_gpu(gpu):
+    """P14's closed form u_j = U (j + 1/2) / (ny + tau - 1/2) reached by the CUDA path itself."""
+    ny, nu, U = 12, 0.2, 0.02
+    for aa in (False, True):
+        g = gpu.Lbm(8, ny, 4, nu, 0.0, flags=gpu.bc_flags("bounce_back", "forced_equilibrium", aa=aa))
+        g.set_top_velocity([U, 0.0, 0.0])
+        g.set_init(gpu.INIT_REST, 0.0, 0.0)
+        g.init(1)
+        g.step(int(6 * ny * ny / nu) + 1)
+        _, u = g.get_macros()
+        exact = U * (np.arange(ny) + 0.5) / (ny + 3 * nu)
+        assert np.abs(u[0].cpu().numpy() - exact[None, :, None]).max() <= 2e-5 * U
+
+
+# ---------------------------------------------------------------------------------------------
+# per-cell solid mask (NEXT #2; PAPER.md:L129-135, L226)
+# ---------------------------------------------------------------------------------------------
+def _solid_mask(kind, nx, ny, nz):
+    m = np.zeros((nz, ny, nx), bool)
+    if kind == "random":
+        m = np.random.default_rng(21).uniform(size=m.shape) < 0.12
+    elif kind == "boxes":                     # trip boxes on the ground, one across the x wrap
+        m[1:4, 0:3, 5:9] = True
+        m[2:5, 0:2, nx - 2:] = True
+        m[2:5, 0:2, :2] = True
+        m[0, 4:6, 30:34] = True               # straddles a 32-cell mask word
+    elif kind == "top":
+        m[:, -1, ::3] = True                  # solids in the row under the free-slip face
+    return m
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("kind", ["random", "boxes", "top"])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (96, 4), (64, 2), (32, 1)])
+def test_solid_mask_parity(orc, gpu, aa, kind, nx, vec):
+    cfg = wl.small(nx=nx, ny=10, nz=6)
+    cfg["solid"] = _solid_mask(kind, nx, 10, 6)
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    assert _state_err(o, g, w) <= 5e-8
+    o.stats_accumulate(1)
+    g.stats_accumulate(1)
+    g.stats_reset()
+    o.stats_reset()
+    for n in (1, 1, 2, 7):                    # odd and even step counts: both AA parities
+        o.step(n)
+        g.step(n)
+        assert _state_err(o, g, w) <= 2e-7
+        er, eu = _macro_err(o, g)
+        assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+    so, no = o.stats_read()
+    sg, ng = g.stats_read()
+    assert no == ng == 11
+    _check_stats(sg, so, cfg["u_bulk"])
+    rg, ug = g.get_macros()
+    solid = cfg["solid"]
+    assert np.all(rg.cpu().numpy()[solid] == 1.0) and np.all(ug.cpu().numpy()[:, solid] == 0.0)
+
+
+def test_solid_mask_needs_nx_multiple_of_32(gpu):
+    with pytest.raises(gpu.LbmError) as e:
+        gpu.Lbm(36, 4, 4, 0.01, 0.1, flags=gpu.bc_flags("bounce_back", "free_slip", solid=True))
+    assert e.value.code == gpu.LBM_EINVAL
+
+
+def test_set_solid_requires_reinit(gpu):
+    g = gpu.Lbm(32, 4, 4, 0.01, 0.1, flags=gpu.bc_flags("bounce_back", "free_slip", solid=True))
+    g.set_init(gpu.INIT_REST, 0.0, 0.0)
+    g.init(1)
+    g.step(1)
+    g.set_solid(np.zeros((4, 4, 32), bool))
+    with pytest.raises(gpu.LbmError) as e:
+        g.step(1)
+    assert e.value.code == gpu.LBM_ESTATE
+
+
 def test_step_before_init_is_an_error(gpu):
     g = gpu.Lbm(8, 4, 4, 0.01, 0.1)
     with pytest.raises(gpu.LbmError) as e:

@@ -65,7 +65,16 @@ def test_create_argument_errors(lb):
     assert create(nx=0) == lb.LBM_EINVAL
     assert create(nx=4096, ny=1024, nz=1024) == lb.LBM_EINVAL          # >= 2^31 cells
     assert create(flags=lb.BOTTOM_PERIODIC | lb.TOP_WALL) == lb.LBM_EINVAL  # periodic-y needs both
-    assert create(flags=3 << 2) == lb.LBM_EINVAL                        # forced-eq top: not built
+    assert create(flags=lb.BOTTOM_PERIODIC | lb.TOP_FORCED_EQ) == lb.LBM_EINVAL  # lid needs a wall below
+    assert create(flags=lb.TOP_FORCED_EQ) == lb.LBM_OK
+    utop = (C.c_double * 3)(0.05, 0.0, 0.0)
+    assert L.lbm_set_top_velocity(h, C.cast(utop, dp)) == lb.LBM_OK
+    utop[1] = float("nan")
+    assert L.lbm_set_top_velocity(h, C.cast(utop, dp)) == lb.LBM_EINVAL
+    L.lbm_destroy(h)
+    assert create() == lb.LBM_OK
+    assert L.lbm_set_top_velocity(h, C.cast(utop, dp)) == lb.LBM_EINVAL   # not a lid handle
+    L.lbm_destroy(h)
     assert create(nx=6, flags=4 << 8) == lb.LBM_EINVAL                  # vec=4 does not divide 6
     assert create(flags=1 << 20) == lb.LBM_EINVAL
     bad = (C.c_double * 8)(*([0.1] * 7 + [-1.0]))
@@ -126,3 +135,33 @@ def test_no_cpu_fallback(lb):
         pytest.skip("GPU present")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         lb.Lbm(8, 8, 8, 0.01, 0.1)
+
+
+def test_normalisation_helpers_closed_forms(lb):
+    """NEXT #3 host helpers against the paper's definitions (L179 Eq. 16) and Table I."""
+    import os
+    g = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_table1.txt")):
+        if not line.startswith("#") and line.strip():
+            k, v = line.split()
+            g[k] = float(v)
+    u_tau = lb.wall_friction_velocity(g["F"], g["H"], 1.0)
+    assert u_tau * g["H"] / g["nu"] == pytest.approx(177.6, abs=0.1)       # Table I => Re_tau = 177.6
+    ny, h = 20, 4
+    st = np.zeros((ny, lb.NSTAT))
+    st[:, 0] = np.linspace(0.01, 0.08, ny)
+    st[:, 3] = 4e-6; st[:, 4] = 1e-6; st[:, 5] = -1e-12                    # tiny negative variance -> 0
+    st[:, 6] = -np.arange(ny) * 1e-6
+    st[:, 7] = 2e-6
+    st[:, 9] = 1.0
+    uv = -0.5 * (7 + 8) * 1e-6
+    assert lb.forest_friction_velocity(st, h) == pytest.approx((uv ** 2 + (2e-6) ** 2) ** 0.25, rel=1e-14)
+    with pytest.raises(lb.LbmError):
+        lb.forest_friction_velocity(st, 10)                                # 2h = ny
+    n = lb.stats_normalise(st, 0.002)
+    assert np.allclose(n[:, 0], st[:, 0] / 0.002) and np.allclose(n[:, 3], 1.0) and np.allclose(n[:, 4], 0.5)
+    assert np.all(n[:, 5] == 0.0) and np.allclose(n[:, 6], st[:, 6] / 4e-6) and np.all(n[:, 9] == 1.0)
+    with pytest.raises(lb.LbmError):
+        lb.stats_normalise(st, 0.0)
+    yp = lb.wall_units(4, 0.01, 2e-4)
+    assert np.allclose(yp, (np.arange(4) + 0.5) * 50.0)

@@ -480,3 +480,128 @@ def test_create_rejects_bad_arguments(orc):
         orc.Oracle(4, 4, 4, -1.0, 0.1)
     with pytest.raises(ValueError):
         orc.Oracle(4, 4, 4, 1e-3, 0.1, bc=orc.BOTTOM_PERIODIC | orc.TOP_WALL)
+
+
+# ---------------------------------------------------------------------------------------------
+# P14 forced-equilibrium lid: steady Couette flow
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ny,nu,U", [(12, 0.05, 0.05), (16, 0.2, 0.02)])
+def test_p14_couette_under_forced_equilibrium_lid(orc, ny, nu, U):
+    """Wall at rest below, lid populations f_eq(1, U e_x) above, Cs = 0, no force.  In a steady
+    linear shear of slope s the first-order non-equilibrium part is f_neq,i = -3 tau w_i c_ix c_iy s,
+    so a population arriving from the row above, f_eq,i(u_{j+1}) + (1 - 1/tau) f_neq,i, equals (to
+    first order in u, which is all that carries x momentum) an equilibrium at u_j + tau s.  The lid
+    supplies an equilibrium at U, hence U = u_{ny-1} + tau s; with the halfway wall below,
+    u_j = s (j + 1/2), this gives the closed form  u_j = U (j + 1/2) / (ny + tau - 1/2)."""
+    o = orc.Oracle(4, ny, 4, nu, 0.0, (0.0, 0.0, 0.0), 0.0, None,
+                   orc.bc_flags("bounce_back", "forced_equilibrium"))
+    o.set_top_velocity([U, 0.0, 0.0])
+    o.init(2, 0.0, 0.0, 1)
+    o.step(int(6 * ny * ny / nu))
+    rho, u = o.get_macros()
+    tau = 3.0 * nu + 0.5
+    exact = U * (np.arange(ny) + 0.5) / (ny + tau - 0.5)
+    assert np.abs(u[0] - exact[None, :, None]).max() <= 1e-9 * U
+    assert np.abs(u[1:]).max() <= 1e-12 and np.abs(rho - 1.0).max() <= 1e-9
+    # a wrong lid (e.g. bounce-back, or equilibrium at rest) gives u = 0 everywhere
+    assert u[0, 0, -1, 0] > 0.9 * U * (ny - 0.5) / (ny + 1.0)
+
+
+def test_p14_lid_at_rest_keeps_rest_state(orc):
+    o = orc.Oracle(6, 5, 4, 0.01, 0.1, (0.0, 0.0, 0.0), 0.0, None,
+                   orc.bc_flags("bounce_back", "forced_equilibrium"))
+    o.init(2, 0.0, 0.0, 1)
+    o.step(200)
+    _, w, _, _ = orc.tables()
+    assert np.abs(o.get_populations() - w[:, None, None, None]).max() <= 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# P15 per-cell solid mask (SURVEY.md §8(f) NEXT #2; PAPER.md:L129-135, L226)
+# ---------------------------------------------------------------------------------------------
+def _push_stream_solid(f, c, opp, mir, bottom, top, solid):
+    """PUSH formulation with solid cells: a population whose landing cell is solid returns into
+    its source cell reversed; nothing leaves a solid cell (it keeps its own values)."""
+    Q, nz, ny, nx = f.shape
+    out = np.full_like(f, np.nan)
+    for z in range(nz):
+        for y in range(ny):
+            for x in range(nx):
+                if solid[z, y, x]:
+                    out[:, z, y, x] = f[:, z, y, x]
+                    continue
+                for i in range(Q):
+                    xd, yd, zd = (x + c[i, 0]) % nx, y + c[i, 1], (z + c[i, 2]) % nz
+                    j = i
+                    if yd < 0:
+                        if bottom == "periodic":
+                            yd = ny - 1
+                        else:
+                            xd, yd, zd, j = x, y, z, opp[i]
+                    elif yd >= ny:
+                        if top == "periodic":
+                            yd = 0
+                        elif top == "free_slip":
+                            yd, j = y, mir[i]
+                        else:
+                            xd, yd, zd, j = x, y, z, opp[i]
+                    if solid[zd, yd, xd]:
+                        xd, yd, zd, j = x, y, z, opp[i]
+                    assert np.isnan(out[j, zd, yd, xd])
+                    out[j, zd, yd, xd] = f[i, z, y, x]
+    assert not np.isnan(out).any()
+    return out
+
+
+@pytest.mark.parametrize("bottom,top", [("bounce_back", "bounce_back"), ("bounce_back", "free_slip"),
+                                        ("periodic", "periodic")])
+def test_p15_stream_with_random_solids_against_brute_force_push(orc, bottom, top):
+    nx, ny, nz = 6, 5, 4
+    c, w, opp, mir = orc.tables()
+    rng = np.random.default_rng(15)
+    solid = rng.uniform(size=(nz, ny, nx)) < 0.2
+    o = orc.Oracle(nx, ny, nz, 1e-3, 0.1, (0, 0, 0), 0.0, None, orc.bc_flags(bottom, top, solid=True))
+    f = rng.uniform(0.01, 1.0, (19, nz, ny, nx))
+    o.set_populations(f)
+    o.set_solid(solid)
+    f = o.get_populations()                 # set_solid puts the rest state into the solid cells
+    assert np.array_equal(f[:, solid], np.broadcast_to(w[:, None], f[:, solid].shape))
+    assert np.array_equal(o.stream_only(), _push_stream_solid(f, c, opp, mir, bottom, top, solid))
+
+
+def test_p15_solid_layers_equal_wall_faces(orc):
+    """A channel whose outer rows are solid is the same problem as a shorter channel between
+    wall faces: the fluid rows agree to rounding, with force, canopy and Smagorinsky on."""
+    nx, ny, nz, pad = 8, 9, 6, 2
+    lad = np.zeros(ny); lad[:3] = 0.1
+    a = orc.Oracle(nx, ny, nz, 1e-3, 0.1, (2e-6, 0, 0), 0.2, lad, orc.bc_flags("bounce_back", "bounce_back"))
+    ladb = np.zeros(ny + 2 * pad); ladb[pad:pad + ny] = lad
+    b = orc.Oracle(nx, ny + 2 * pad, nz, 1e-3, 0.1, (2e-6, 0, 0), 0.2, ladb,
+                   orc.bc_flags("bounce_back", "bounce_back", solid=True))
+    rho, u = a.init_field(0, 0.05, 0.05, 99)
+    a.set_macros(rho, u)
+    rb = np.ones((nz, ny + 2 * pad, nx)); ub = np.zeros((3, nz, ny + 2 * pad, nx))
+    rb[:, pad:pad + ny] = rho; ub[:, :, pad:pad + ny] = u
+    b.set_macros(rb, ub)
+    solid = np.zeros((nz, ny + 2 * pad, nx), bool); solid[:, :pad] = True; solid[:, pad + ny:] = True
+    b.set_solid(solid)
+    a.step(60); b.step(60)
+    fa, fb = a.get_populations(), b.get_populations()
+    assert np.abs(fb[:, :, pad:pad + ny] - fa).max() <= 1e-15
+    ra, ua = a.get_macros(); r2, u2 = b.get_macros()
+    assert np.abs(u2[:, :, pad:pad + ny] - ua).max() <= 1e-15
+    assert np.all(r2[solid] == 1.0) and np.all(u2[:, solid] == 0.0)
+
+
+def test_p15_mass_conserved_with_solids(orc):
+    cfg = wl.small(16, 10, 8)
+    rng = np.random.default_rng(5)
+    solid = rng.uniform(size=(8, 10, 16)) < 0.1
+    o = orc.Oracle(16, 10, 8, cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                   orc.lad_from_spec(cfg["forest"], 10), orc.bc_flags("bounce_back", "free_slip", solid=True))
+    o.init(0, 0.05, 0.05, 3)
+    o.set_solid(solid)
+    m0 = o.get_populations()[:, ~solid].sum()
+    o.step(300)
+    m1 = o.get_populations()[:, ~solid].sum()
+    assert abs(m1 - m0) <= 1e-12 * m0
