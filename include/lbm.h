@@ -125,6 +125,12 @@ int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host);
  * plane sums and the stage-2 reduction kernel on sampled steps).  Asynchronous. */
 int lbm_step(lbm_t *h, int n);
 
+/* CUDA graphs for launch-bound lattices: with graphs on, lbm_step(n) replays blocks of about 32
+ * time steps as one captured graph of the same kernel launches (bit-identical results) and runs
+ * the remainder directly.  mode 0 off, 1 on, 2 auto (default: on for lattices of at most 2^22
+ * cells).  Not used while kernel timing is on or while the caller is capturing the stream. */
+int lbm_set_graphs(lbm_t *h, int mode);
+
 /* Sample S_k of the current state (see "Time" above) into caller-owned buffers (layouts as in
  * lbm_set_macros).  Either pointer may be NULL.  _dev is asynchronous; _host synchronises. */
 int lbm_get_macros(lbm_t *h, float *rho_dev, float *u_dev);

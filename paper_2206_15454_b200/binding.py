@@ -38,7 +38,7 @@ SYMBOLS = [
     "lbm_launch_count", "lbm_set_launch_shape", "lbm_variant", "lbm_destroy", "lbm_last_error",
     "lbm_lad_profile", "lbm_mix64", "lbm_set_kernel_timing", "lbm_kernel_timing_read",
     "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
-    "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units",
+    "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs",
 ]
 
 
@@ -65,6 +65,7 @@ def lib():
         L.lbm_set_init.argtypes = [vp, C.c_int, C.c_double, C.c_double]
         L.lbm_set_top_velocity.argtypes = [vp, dp]
         L.lbm_set_solid.argtypes = [vp, C.c_void_p]
+        L.lbm_set_graphs.argtypes = [vp, C.c_int]
         L.lbm_wall_friction_velocity.argtypes = [C.c_double, C.c_double, C.c_double, dp]
         L.lbm_forest_friction_velocity.argtypes = [dp, C.c_int, C.c_int, dp]
         L.lbm_stats_normalise.argtypes = [dp, C.c_int, C.c_double, dp]
@@ -343,6 +344,10 @@ class Lbm:
         n = C.c_longlong(0)
         _check(lib().lbm_stats_read(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
         return out, int(n.value)
+
+    def set_graphs(self, mode: int):
+        """0 off, 1 on, 2 auto (CUDA graphs of ~32 steps inside lbm_step)."""
+        _check(lib().lbm_set_graphs(self._h, int(mode)))
 
     def set_kernel_timing(self, on: bool):
         _check(lib().lbm_set_kernel_timing(self._h, int(bool(on))))

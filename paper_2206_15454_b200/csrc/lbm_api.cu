@@ -87,11 +87,22 @@ struct lbm_s {
     double U_ref, noise_frac;
     char variant[64];
     KParams kp;
+    // CUDA graph of G consecutive steps (launch-bound small lattices)
+    int graph_mode;              // 0 off, 1 on, 2 auto (small lattices only)
+    cudaGraphExec_t gexec;       // nullptr = none cached
+    int g_steps, g_parity, g_every;
+    long long g_launches, g_samples;
     bool timing;
     std::vector<cudaEvent_t> ev; // start/stop pairs of the bracketed step-kernel launches
     size_t ev_used;
 };
 constexpr size_t MAX_TIMED = 4096;
+
+static void graph_drop(lbm_s *h)
+{
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    h->gexec = nullptr;
+}
 
 static bool valid_top_bottom(uint32_t bc, int *bot, int *top)
 {
@@ -192,6 +203,8 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
     h->init_kind = LBM_INIT_REST; h->U_ref = 0.0; h->noise_frac = 0.0;
     h->timing = false; h->ev_used = 0;
+    h->graph_mode = 2; h->gexec = nullptr; h->g_steps = 0; h->g_parity = 0; h->g_every = 0;
+    h->g_launches = 0; h->g_samples = 0;
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
     snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", V, h->TX, h->TY);
     *out = h;
@@ -206,6 +219,7 @@ int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
         ((long long)h->ny * h->nz) % ty)
         return fail(LBM_EINVAL, "launch shape %dx%d does not tile %d thread columns x %lld rows", tx, ty, W,
                     (long long)h->ny * h->nz);
+    graph_drop(h);
     h->TX = tx; h->TY = ty; h->nchunk = W / tx;
     h->kp.nchunk = h->nchunk;
     snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", h->V, h->TX, h->TY);
@@ -223,6 +237,8 @@ static void fill_params(lbm_s *h)
     p.tau0 = (float)tau0; p.tau0sq = (float)(tau0 * tau0);
     p.ksmag = (float)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs); // R9: C_smag = Cs^2
     p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
+    // the fp64 momentum channel adds the same (fp32-rounded) force the fp32 terms use
+    p.Fb64[0] = (double)p.Fbx; p.Fb64[1] = (double)p.Fby; p.Fb64[2] = (double)p.Fbz;
     p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
     {
@@ -249,6 +265,7 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     if (!dev_workspace) return fail(LBM_EINVAL, "workspace is NULL");
     if (bytes < h->L.total) return fail(LBM_ENOMEM, "workspace too small: %zu < %zu bytes", bytes, h->L.total);
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) return fail(LBM_ENOMEM, "workspace must be 256-byte aligned");
+    graph_drop(h);
     h->ws = static_cast<char *>(dev_workspace);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
     fill_params(h);
@@ -297,6 +314,7 @@ int lbm_set_top_velocity(lbm_t *h, const double *U_top)
     for (int a = 0; a < 3; ++a)
         if (!std::isfinite(U_top[a])) return fail(LBM_EINVAL, "U_top[%d] is not finite", a);
     for (int a = 0; a < 3; ++a) h->Utop[a] = U_top[a];
+    graph_drop(h);
     if (h->bound) fill_params(h);
     return LBM_OK;
 }
@@ -480,11 +498,9 @@ int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host)
     return LBM_OK;
 }
 
-int lbm_step(lbm_t *h, int n)
+// n time steps, one launch (+ the stage-2 launch on sampled steps) each
+static int step_direct(lbm_s *h, int n)
 {
-    if (!h) return fail(LBM_EINVAL, "handle is NULL");
-    if (!h->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init / lbm_set_macros");
-    if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
     for (int k = 0; k < n; ++k) {
         const bool sample = h->stats_every > 0 && (h->stats_phase % h->stats_every) == 0;
         KParams p = h->kp;
@@ -514,6 +530,89 @@ int lbm_step(lbm_t *h, int n)
         if (h->stats_every > 0) h->stats_phase++;
         h->t++;
     }
+    return LBM_OK;
+}
+
+// Steps per graph: a whole number of periods of (storage parity x sampling cadence), about 32
+// steps; 0 = this cadence is not worth a graph.
+static int graph_span(const lbm_s *h)
+{
+    const int e = h->stats_every;
+    const int period = (e == 0) ? 2 : ((e % 2 == 0) ? e : 2 * e);
+    if (period > 64) return 0;
+    int reps = 32 / period;
+    if (reps < 1) reps = 1;
+    return period * reps;
+}
+
+// Capture G steps starting at the current parity (sampling phase 0) into an executable graph.
+// Returns LBM_OK with h->gexec == nullptr when the stream cannot be captured (e.g. the caller
+// is capturing it already): the caller then falls back to direct launches.
+static int graph_build(lbm_s *h, int G)
+{
+    graph_drop(h);
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(h->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return LBM_OK;
+    }
+    const long long t0 = h->t, ph0 = h->stats_phase, ns0 = h->nsamples, l0 = h->launches;
+    if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return LBM_OK;
+    }
+    const int rc = step_direct(h, G);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+    h->g_launches = h->launches - l0; h->g_samples = h->nsamples - ns0;
+    h->t = t0; h->stats_phase = ph0; h->nsamples = ns0; h->launches = l0;   // nothing has run yet
+    if (rc != LBM_OK || e != cudaSuccess || !graph) {
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        return LBM_OK;
+    }
+    if (cudaGraphInstantiate(&h->gexec, graph, 0) != cudaSuccess) { cudaGetLastError(); h->gexec = nullptr; }
+    cudaGraphDestroy(graph);
+    h->g_steps = G; h->g_parity = (int)(t0 & 1); h->g_every = h->stats_every;
+    return LBM_OK;
+}
+
+int lbm_step(lbm_t *h, int n)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init / lbm_set_macros");
+    if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
+    // small lattices are launch-bound: replay G steps as one CUDA graph (identical kernels and
+    // order, so results are bit-identical to direct launches)
+    const bool want = h->graph_mode == 1 || (h->graph_mode == 2 && h->N <= (1ll << 22));
+    const int G = (want && !h->timing) ? graph_span(h) : 0;
+    if (G > 0 && n >= 2 * G) {
+        if (h->stats_every > 0) {            // align the sampling phase first
+            const int mis = (int)(h->stats_phase % h->stats_every);
+            if (mis) { const int a = h->stats_every - mis; int rc = step_direct(h, a); if (rc) return rc; n -= a; }
+        }
+        if (n >= G) {
+            if (!h->gexec || h->g_steps != G || h->g_parity != (int)(h->t & 1) || h->g_every != h->stats_every) {
+                int rc = graph_build(h, G);
+                if (rc) return rc;
+            }
+            while (h->gexec && n >= G) {
+                CU_TRY(cudaGraphLaunch(h->gexec, h->stream));
+                h->t += G; h->launches += h->g_launches; h->nsamples += h->g_samples;
+                if (h->stats_every > 0) h->stats_phase += G;
+                n -= G;
+            }
+        }
+    }
+    return step_direct(h, n);
+}
+
+int lbm_set_graphs(lbm_t *h, int mode)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (mode < 0 || mode > 2) return fail(LBM_EINVAL, "mode must be 0 (off), 1 (on) or 2 (auto)");
+    h->graph_mode = mode;
+    if (mode == 0) graph_drop(h);
     return LBM_OK;
 }
 
@@ -651,6 +750,7 @@ int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches)
 void lbm_destroy(lbm_t *h)
 {
     if (!h) return;
+    graph_drop(h);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
     delete h;
 }

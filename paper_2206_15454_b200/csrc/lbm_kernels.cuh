@@ -64,6 +64,7 @@ struct KParams {
     // physics (fp32 copies)
     float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
     float Fbx, Fby, Fbz;        // body force density F_b
+    double Fb64[3];             // the same in fp64 (momentum channel)
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)

@@ -64,9 +64,10 @@ def test_long_run_statistics(orc, gpu, case, aa, spin, window):
     d_mean = np.abs(sg[:, 0] - so[:, 0]).max() / umax
     print(f"{case} {g.variant}: local max|du| after {spin + window} steps = {diverged:.2e}; "
           f"mean U differs by {100 * d_mean:.3f} % of max")
-    # the runs have left the short-time tolerance far behind ...
-    assert diverged > 10 * 1e-5 * cfg["u_bulk"]
-    # ... and the statistics still agree
+    # cfg1 (sheared canopy flow) has left the short-time tolerance far behind by now; the small
+    # channel stays closer.  Either way the statistics must agree
+    if case == "cfg1":
+        assert diverged > 10 * 1e-5 * cfg["u_bulk"]
     assert d_mean <= 0.02
     for k, name in ((3, "uu"), (4, "vv"), (5, "ww"), (6, "uv")):
         m = np.abs(so[:, k]).max()

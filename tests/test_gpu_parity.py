@@ -102,6 +102,27 @@ def test_vector_drag_and_general_force(orc, gpu, aa):
     assert _state_err(o, g, w) <= 2e-7
 
 
+@pytest.mark.parametrize("shape", [(1, 1, 1), (4, 1, 1), (1, 5, 1), (2, 3, 1), (8, 1, 7), (5, 2, 3), (3, 1, 3),
+                                   (1, 1, 6), (12, 2, 1)])
+@pytest.mark.parametrize("bottom,top", BCS, ids=["wall-slip", "wall-wall", "periodic"])
+def test_degenerate_lattices(orc, gpu, shape, bottom, top):
+    """One-cell-thick lattices: the periodic wrap lands on the cell itself, one row touches both
+    y faces at once.  Both storage schemes, odd and even step counts."""
+    nx, ny, nz = shape
+    cfg = wl.small(nx=nx, ny=ny, nz=nz, bottom=bottom, top=top, forest_rows=min(1, ny))
+    w = _weights(orc)
+    for aa in (False, True):
+        o, g = _pair(orc, gpu, cfg, aa, 0)
+        assert _state_err(o, g, w) <= 5e-8
+        for n in (1, 2, 0, 5):
+            o.step(n)
+            g.step(n)
+            assert _state_err(o, g, w) <= 2e-7, (aa, n)
+        er, eu = _macro_err(o, g)
+        assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+        assert g.time == 8
+
+
 def test_single_block_shapes(orc, gpu):
     """Different thread-block shapes (row split across blocks, several rows per block) agree."""
     cfg = wl.small(nx=256, ny=8, nz=4)
@@ -389,6 +410,36 @@ def test_set_solid_requires_reinit(gpu):
     with pytest.raises(gpu.LbmError) as e:
         g.step(1)
     assert e.value.code == gpu.LBM_ESTATE
+
+
+# ---------------------------------------------------------------------------------------------
+# CUDA-graph replay inside lbm_step: same kernels in the same order => bit-identical
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("every", [0, 1, 3, 4])
+def test_graph_replay_is_bit_identical(gpu, aa, every):
+    import torch
+    cfg = wl.get("cfg1")
+    out = []
+    for mode in (0, 1):
+        g = gpu.Lbm.from_config(cfg, aa=aa)
+        g.set_graphs(mode)
+        g.init(cfg["seed"])
+        g.step(1)                               # start from an odd time step
+        g.stats_accumulate(every)
+        l0 = g.launch_count
+        g.step(2)                               # put the sampling phase out of alignment
+        g.step(203)
+        g.step(77)                              # a second call reuses or rebuilds the graph
+        st = g.get_state()
+        s, n = g.stats_read()
+        torch.cuda.synchronize()
+        out.append((st.cpu().numpy(), s, n, g.time, g.launch_count - l0))
+        g.close()
+    (sa, ta, na, tia, la), (sb, tb, nb, tib, lbb) = out
+    assert tia == tib == 283 and na == nb == (0 if every == 0 else -(-282 // every))
+    assert la == lbb                             # launches replayed through a graph are counted
+    assert np.array_equal(sa, sb) and np.array_equal(ta, tb)
 
 
 def test_step_before_init_is_an_error(gpu):

@@ -81,6 +81,8 @@ def test_create_argument_errors(lb):
     assert create(lad=C.cast(bad, dp)) == lb.LBM_EINVAL
     # calls out of order never touch the GPU
     assert create() == lb.LBM_OK
+    assert L.lbm_set_graphs(h, 3) == lb.LBM_EINVAL and L.lbm_set_graphs(h, 1) == lb.LBM_OK
+    assert L.lbm_set_solid(h, None) == lb.LBM_EINVAL                     # not a mask handle
     assert L.lbm_step(h, 1) == lb.LBM_ESTATE
     assert L.lbm_init(h, 1) == lb.LBM_ESTATE
     assert L.lbm_bind(h, None, 0, None) == lb.LBM_EINVAL
