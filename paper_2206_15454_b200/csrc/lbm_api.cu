@@ -37,7 +37,7 @@ constexpr int MAX_NCHUNK = 8;
 constexpr size_t STAGING_BUDGET = (size_t)256 << 20;
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, solid, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, solid, solid_nb, staging, total;
     int stage_planes;
 };
 
@@ -55,6 +55,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     L.uprof = off; off = align_up(off + (size_t)ny * 4, 256);
     L.flag = off; off += 256;
     L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
+    L.solid_nb = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     const size_t plane = (size_t)16 * nx * ny;
     size_t planes = STAGING_BUDGET / plane;
     if (planes < 1) planes = 1;
@@ -253,6 +254,7 @@ static void fill_params(lbm_s *h)
         }
     }
     p.solid = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid) : nullptr;
+    p.solid_nb = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid_nb) : nullptr;
     p.nxw = (h->nx + 31) / 32;
     p.partial = nullptr; p.shift = nullptr;
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
@@ -275,8 +277,11 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
-    if (h->mask)
-        CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4, h->stream));
+    if (h->mask) {
+        const size_t mbytes = (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4;
+        CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, mbytes, h->stream));
+        CU_TRY(cudaMemsetAsync(h->ws + h->L.solid_nb, 0, mbytes, h->stream));
+    }
     CU_TRY(cudaStreamSynchronize(h->stream)); // cda is a local vector
     h->bound = true; h->inited = false;
     return LBM_OK;
@@ -300,7 +305,28 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
                 for (int x = 0; x < h->nx; ++x)
                     if (row[x]) { out[x >> 5] |= 1u << (x & 31); h->nfluid[y] -= 1.0; }
             }
+    // the mask dilated by one cell in every direction (periodic x, z; y only where periodic):
+    // bit = some cell within one step is solid.  The kernels skip the geometry work where it is 0.
+    std::vector<uint32_t> nb;
+    try { nb.assign(words, 0u); } catch (...) { return fail(LBM_ENOMEM, "host allocation failed"); }
+    const bool yper = h->bot == BC_BOT_PERIODIC;
+    for (int z = 0; z < h->nz; ++z)
+        for (int y = 0; y < h->ny; ++y) {
+            uint32_t *out = nb.data() + ((size_t)z * h->ny + y) * nxw;
+            for (int dz = -1; dz <= 1; ++dz)
+                for (int dy = -1; dy <= 1; ++dy) {
+                    int yy = y + dy;
+                    if (yy < 0 || yy >= h->ny) { if (!yper) continue; yy = (yy + h->ny) % h->ny; }
+                    const int zz = (z + dz + h->nz) % h->nz;
+                    const uint32_t *row = bits.data() + ((size_t)zz * h->ny + yy) * nxw;
+                    for (int w = 0; w < nxw; ++w) {
+                        const uint32_t m = row[w], l = row[w == 0 ? nxw - 1 : w - 1], r = row[w + 1 == nxw ? 0 : w + 1];
+                        out[w] |= m | (m << 1) | (m >> 1) | (l >> 31) | (r << 31);
+                    }
+                }
+        }
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid_nb, nb.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream));
     h->inited = false;   // the populations must be rebuilt around the new geometry
     return LBM_OK;

@@ -68,6 +68,7 @@ struct KParams {
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
+    const unsigned *solid_nb;   // the same mask dilated by one cell in x, y, z (host-built)
     int nxw;                    // words per x row (nx / 32)
     float lid[5];               // forced-equilibrium lid: f_eq,i(1, U_top) - w_i for i = 4, 8, 9, 16, 18
     // statistics
@@ -322,9 +323,17 @@ __device__ __forceinline__ unsigned solid_field(const KParams &p, const Ctx &c, 
     return f;
 }
 
-template <int V>
-__device__ __forceinline__ unsigned long long solid_gather(const KParams &p, const Ctx &c)
+// one word of the dilated mask tells whether any cell within one step of the own cells is solid
+__device__ __forceinline__ unsigned solid_nb_word(const KParams &p, const Ctx &c)
 {
+    return __ldg(p.solid_nb + (long long)(c.y + p.ny * c.z) * p.nxw + (c.x0 >> 5));
+}
+
+template <int V>
+__device__ __forceinline__ unsigned long long solid_gather(const KParams &p, const Ctx &c, unsigned nb)
+{
+    // if no cell within one step is solid every field is zero and the nine-row gather is skipped
+    if (((nb >> (c.x0 & 31)) & ((1u << V) - 1u)) == 0u) return 0ull;
     const int ys[3] = {c.ym, c.y, c.yp}, zs[3] = {c.zm, c.z, c.zp};
     unsigned long long S = 0ull;
 #pragma unroll
@@ -344,35 +353,44 @@ template <int V> __device__ __forceinline__ unsigned solid_self(unsigned long lo
     return (solid_pick(S, 1, 1) >> 1) & ((1u << V) - 1u);
 }
 
-template <int V, int RM, bool MASK>
-__device__ __forceinline__ void load_all(const KParams &p, const Ctx &c, float (&g)[Q][V],
-                                         unsigned long long S = 0ull)
+template <int V, int RM>
+__device__ __forceinline__ void load_all(const KParams &p, const Ctx &c, float (&g)[Q][V])
 {
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
         load_dir<V, RM, i>(p, c, g[i]);
-        if constexpr (MASK && RM != RD_LOCAL && i != 0) {
-            // source cells of this link: (x0+k - c_x) in the row load_dir used
-            bool bb = false, fs = false;
-            if constexpr (cy == 1) bb = c.bot_bb;
-            if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
-            const int a = (bb || fs) ? 1 : 1 - cy, b = bb ? 1 : 1 - cz;
-            const unsigned bits = bb ? 0u : (solid_pick(S, a, b) >> (1 - cx)) & ((1u << V) - 1u);
-            if (bits) {                      // bounce back off the solid neighbour (own cell)
-                constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[i] : i;
-                float own[V];
-                ldv<V>(p.src + (long long)S_BB * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), own);
-#pragma unroll
-                for (int k = 0; k < V; ++k)
-                    if ((bits >> k) & 1u) g[i][k] = own[k];
-            }
-        }
-        if constexpr (cy == -1) {
+        if constexpr (Lat::cy[i] == -1) {
             if (c.top_lid) {
 #pragma unroll
                 for (int k = 0; k < V; ++k) g[i][k] = p.lid[lid_index(i)];
             }
+        }
+    });
+}
+
+// Solid-mask correction of the streamed populations, applied after load_all (so that the 19
+// loads do not wait for the mask): a link whose source cell (x0+k - c_x, in the row load_dir
+// used) is solid bounces back, i.e. takes the own cell's opposite-slot value.
+template <int V, int RM>
+__device__ __forceinline__ void solid_fix_loads(const KParams &p, const Ctx &c, float (&g)[Q][V],
+                                                unsigned long long S)
+{
+    if constexpr (RM == RD_LOCAL) return;
+    static_for<1, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
+        bool bb = false, fs = false;
+        if constexpr (cy == 1) bb = c.bot_bb;
+        if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
+        const int a = (bb || fs) ? 1 : 1 - cy, b = bb ? 1 : 1 - cz;
+        const unsigned bits = bb ? 0u : (solid_pick(S, a, b) >> (1 - cx)) & ((1u << V) - 1u);
+        if (bits) {
+            constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[i] : i;
+            float own[V];
+            ldv<V>(p.src + (long long)S_BB * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), own);
+#pragma unroll
+            for (int k = 0; k < V; ++k)
+                if ((bits >> k) & 1u) g[i][k] = own[k];
         }
     });
 }
@@ -690,10 +708,22 @@ template <int V, int RM, int WM, bool STATS, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, 0);
-    unsigned long long S = 0ull;
-    if constexpr (MASK) S = solid_gather<V>(p, c);
+    // With a mask, a warp none of whose lanes has a solid cell within one step (the usual case:
+    // geometry is sparse) runs the unmasked load/store code; the decision is warp-uniform, so the
+    // full-mask shuffles inside load_dir/store_dir stay converged.
+    // (the mask word is requested first and looked at only after the 19 population loads have
+    // been issued, so it adds no latency to them)
+    unsigned nbw = 0u;
+    if constexpr (MASK) nbw = solid_nb_word(p, c);
     float g[Q][V];
-    load_all<V, RM, MASK>(p, c, g, S);
+    load_all<V, RM>(p, c, g);
+    unsigned long long S = 0ull;
+    bool geom = false;
+    if constexpr (MASK) {
+        S = solid_gather<V>(p, c, nbw);
+        geom = __any_sync(0xffffffffu, S != 0ull);
+        if (geom) solid_fix_loads<V, RM>(p, c, g, S);
+    }
     const float cda = __ldg(p.cda + c.y);
     float s[NSTAT];
     if constexpr (STATS) {
@@ -711,7 +741,8 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
         collide<V>(p, g, k, m);
     }
     const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, 0, true) : c;
-    store_all<V, WM, MASK>(p, c2, g, S);
+    if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
+    else store_all<V, WM, false>(p, c2, g);
     if constexpr (STATS) {
         if (p.shift) {
             const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c2.y);
@@ -728,10 +759,13 @@ template <int V, int RM, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
-    unsigned long long S = 0ull;
-    if constexpr (MASK) S = solid_gather<V>(p, c);
     float g[Q][V];
-    load_all<V, RM, MASK>(p, c, g, S);
+    load_all<V, RM>(p, c, g);
+    unsigned long long S = 0ull;
+    if constexpr (MASK) {
+        S = solid_gather<V>(p, c, solid_nb_word(p, c));
+        if (__any_sync(0xffffffffu, S != 0ull)) solid_fix_loads<V, RM>(p, c, g, S);
+    }
     const float cda = __ldg(p.cda + c.y);
     float s[NSTAT];
 #pragma unroll
@@ -778,7 +812,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const K
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
     unsigned long long S = 0ull;
-    if constexpr (MASK) S = solid_gather<V>(p, c);
+    if constexpr (MASK) S = solid_gather<V>(p, c, solid_nb_word(p, c));
     float g[Q][V];
     const long long cell0 = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;

@@ -288,7 +288,9 @@ def _subbox_check(orc, gpu, cfg, aa, boxes, presteps):
     return worst, g
 
 
-@pytest.mark.parametrize("name,aa", [("cfg3", False), ("cfg3", True), ("cfg4", True), ("cfg5", True)])
+@pytest.mark.parametrize("name,aa", [("cfg3", False), ("cfg3", True), ("cfg4", True), ("cfg5", True),
+                                     ("paper_channel", False), ("paper_channel", True),
+                                     ("paper_abl_fine", False), ("paper_abl_fine", True)])
 def test_full_size_sampled_boxes(orc, gpu, name, aa):
     import torch
     cfg = wl.get(name)
@@ -297,7 +299,7 @@ def test_full_size_sampled_boxes(orc, gpu, name, aa):
     if free < need:
         pytest.skip(f"{name} needs {need / 2**30:.0f} GiB of device memory")
     nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
-    h = cfg["forest"]["h"]
+    h = (cfg["forest"] or {}).get("h", (cfg["forest"] or {}).get("rows", 8))
     boxes = [(0, 0, 0), (nx - 4, 0, nz - 4), (nx // 2 - 3, h - 4, nz // 3), (nx - 8, ny - 8, 0),
              (5, ny - 8, nz - 5), (nx // 3, ny // 2, nz // 2), (124, 0, 1), (nx - 5, ny // 4, nz - 3)]
     for presteps in (2, 3):                       # AA: next step is even / odd
