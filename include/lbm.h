@@ -58,6 +58,9 @@ typedef enum lbm_status {
 #define LBM_DRAG_VECTOR       (1u << 4)   /* bit 4: 0 streamwise-only drag (paper, L98/L103), 1 vector */
 #define LBM_SOLID_MASK        (1u << 5)   /* bit 5: a per-cell solid bit mask will be given (lbm_set_solid) */
 #define LBM_STORAGE_AA        (1u << 6)   /* bit 6: 0 two-lattice pull, 1 single-array AA pattern     */
+#define LBM_Z_HALO            (1u << 7)   /* bit 7: z slab of a larger lattice: planes 0 and nz-1 are ghost
+                                             planes filled by the halo calls, planes 1..nz-2 are updated
+                                             (two-lattice storage only)                                     */
 #define LBM_VEC_SHIFT         8           /* bits 8-10: cells per thread override (0 auto, 1, 2, 4)   */
 #define LBM_VEC_MASK          (7u << 8)
 
@@ -124,6 +127,33 @@ int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host);
  * Smagorinsky tau, Guo-forced BGK collision, boundary links, store; plus the fused stage-1
  * plane sums and the stage-2 reduction kernel on sampled steps).  Asynchronous. */
 int lbm_step(lbm_t *h, int n);
+
+/* z-slab decomposition (LBM_Z_HALO; "only information from directly adjacent
+ * points is required").  The handle is created with nz = nz_local + 2.  After
+ * lbm_init / lbm_set_macros* and after every lbm_step(1) the caller exchanges the two faces with
+ * its z neighbours: lbm_halo_pack(side, buf) copies the five populations leaving through the low
+ * (side 0: c_z = -1, plane 1) or high (side 1: c_z = +1, plane nz-2) face into the device buffer
+ * [5][ny][nx] fp32; the neighbour passes the buffer it received to lbm_halo_unpack(side, buf),
+ * side = the side of ITS OWN slab the data enters through (0: ghost plane 0 takes c_z = +1 data,
+ * 1: ghost plane nz-1 takes c_z = -1 data).  All asynchronous on the bound stream.
+ * lbm_set_z_slab tells the synthetic initial field where the slab sits: local plane 0 (the low
+ * ghost) is global plane z_first - 1 of nz_global (periodic).  Statistics and lbm_get_macros
+ * cover the interior planes (ghost-plane entries of lbm_get_macros are meaningless); plane
+ * averages divide by nx*(nz-2).  To combine slabs, sum lbm_stats_read_raw over the ranks and
+ * pass the sums to lbm_stats_from_raw (a slab never uses an accumulation centre). */
+int lbm_set_z_slab(lbm_t *h, int z_first, int nz_global);
+int lbm_halo_bytes(const lbm_t *h, size_t *bytes);
+int lbm_halo_pack(lbm_t *h, int side, float *buf_dev);
+int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev);
+
+/* Raw running sums behind lbm_stats_read, for combining slabs: out_host [ny][LBM_NSTAT] doubles of
+ * sum(u-u0), sum(v-v0), sum(w-w0), the six centred second-moment sums and sum(rho) over the
+ * samples and cells seen so far (column 9 holds sum(rho)); centre_host [ny][3] doubles = (u0, v0, w0) per row (may be NULL);
+ * *count = samples x contributing cells per plane (may be NULL).  Synchronises the stream. */
+int lbm_stats_read_raw(lbm_t *h, double *out_host, double *centre_host, double *count);
+/* Host helper: the [ny][LBM_NSTAT] table of lbm_stats_read from raw sums (column 9 = sum of rho),
+ * an optional centre [ny][3] and the total count; count <= 0 gives zeros. */
+int lbm_stats_from_raw(const double *raw_host, const double *centre_host, int ny, double count, double *out_host);
 
 /* CUDA graphs for launch-bound lattices: with graphs on, lbm_step(n) replays blocks of about 32
  * time steps as one captured graph of the same kernel launches (bit-identical results) and runs

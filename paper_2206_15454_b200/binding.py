@@ -19,6 +19,7 @@ TOP_WALL, TOP_FREE_SLIP, TOP_PERIODIC, TOP_FORCED_EQ = 0 << 2, 1 << 2, 2 << 2, 3
 DRAG_VECTOR = 1 << 4
 SOLID_MASK = 1 << 5
 STORAGE_AA = 1 << 6
+Z_HALO = 1 << 7
 VEC_SHIFT = 8
 NSTAT = 10
 
@@ -38,7 +39,8 @@ SYMBOLS = [
     "lbm_launch_count", "lbm_set_launch_shape", "lbm_variant", "lbm_destroy", "lbm_last_error",
     "lbm_lad_profile", "lbm_mix64", "lbm_set_kernel_timing", "lbm_kernel_timing_read",
     "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
-    "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs",
+    "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
+    "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
 ]
 
 
@@ -66,6 +68,12 @@ def lib():
         L.lbm_set_top_velocity.argtypes = [vp, dp]
         L.lbm_set_solid.argtypes = [vp, C.c_void_p]
         L.lbm_set_graphs.argtypes = [vp, C.c_int]
+        L.lbm_set_z_slab.argtypes = [vp, C.c_int, C.c_int]
+        L.lbm_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+        L.lbm_halo_pack.argtypes = [vp, C.c_int, fp]
+        L.lbm_halo_unpack.argtypes = [vp, C.c_int, fp]
+        L.lbm_stats_read_raw.argtypes = [vp, dp, dp, dp]
+        L.lbm_stats_from_raw.argtypes = [dp, dp, C.c_int, C.c_double, dp]
         L.lbm_wall_friction_velocity.argtypes = [C.c_double, C.c_double, C.c_double, dp]
         L.lbm_forest_friction_velocity.argtypes = [dp, C.c_int, C.c_int, dp]
         L.lbm_stats_normalise.argtypes = [dp, C.c_int, C.c_double, dp]
@@ -105,9 +113,9 @@ def _check(rc: int):
 
 
 def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa: bool = False, vec: int = 0,
-             solid: bool = False) -> int:
+             solid: bool = False, halo: bool = False) -> int:
     return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0) | (STORAGE_AA if aa else 0)
-            | (SOLID_MASK if solid else 0) | (int(vec) << VEC_SHIFT))
+            | (SOLID_MASK if solid else 0) | (Z_HALO if halo else 0) | (int(vec) << VEC_SHIFT))
 
 
 def workspace_bytes(nx: int, ny: int, nz: int, flags: int) -> int:
@@ -150,6 +158,15 @@ def stats_normalise(stats: np.ndarray, u_ref: float) -> np.ndarray:
 def wall_units(ny: int, u_tau: float, nu: float) -> np.ndarray:
     out = np.empty(int(ny))
     _check(lib().lbm_wall_units(int(ny), float(u_tau), float(nu), _dp(out)))
+    return out
+
+
+def stats_from_raw(raw: np.ndarray, count: float, centre=None) -> np.ndarray:
+    """The lbm_stats_read table from (summed) raw sums; see include/lbm.h."""
+    raw = np.ascontiguousarray(raw, dtype=np.float64)
+    out = np.empty_like(raw)
+    cp = None if centre is None else _dp(np.ascontiguousarray(centre, dtype=np.float64))
+    _check(lib().lbm_stats_from_raw(_dp(raw), cp, raw.shape[0], float(count), _dp(out)))
     return out
 
 
@@ -205,11 +222,11 @@ class Lbm:
         _check(L.lbm_bind(self._h, C.c_void_p(aligned), C.c_size_t(nbytes), C.c_void_p(self._stream.cuda_stream)))
 
     @classmethod
-    def from_config(cls, cfg: dict, aa=None, vec: int = 0, **kw) -> "Lbm":
+    def from_config(cls, cfg: dict, aa=None, vec: int = 0, halo: bool = False, **kw) -> "Lbm":
         if aa is None:
             aa = cfg.get("storage", "two_lattice") == "aa"
         flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec,
-                         solid=cfg.get("solid") is not None)
+                         solid=cfg.get("solid") is not None, halo=halo)
         s = cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
                 lad_from_spec(cfg["forest"], cfg["ny"]), flags, **kw)
         i = cfg["init"]
@@ -344,6 +361,33 @@ class Lbm:
         n = C.c_longlong(0)
         _check(lib().lbm_stats_read(self._h, out.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
         return out, int(n.value)
+
+    # ---- z-slab halo mode (LBM_Z_HALO) ----
+    def set_z_slab(self, z_first: int, nz_global: int):
+        _check(lib().lbm_set_z_slab(self._h, int(z_first), int(nz_global)))
+
+    def halo_buffer(self):
+        """A CUDA tensor of the size lbm_halo_pack / lbm_halo_unpack move: (5, ny, nx) float32."""
+        import torch
+
+        n = C.c_size_t(0)
+        _check(lib().lbm_halo_bytes(self._h, C.byref(n)))
+        assert n.value == 5 * self.ny * self.nx * 4
+        return torch.empty((5, self.ny, self.nx), dtype=torch.float32, device=self.device)
+
+    def halo_pack(self, side: int, buf):
+        _check(lib().lbm_halo_pack(self._h, int(side), self._dev(buf, (5, self.ny, self.nx))))
+
+    def halo_unpack(self, side: int, buf):
+        _check(lib().lbm_halo_unpack(self._h, int(side), self._dev(buf, (5, self.ny, self.nx))))
+
+    def stats_read_raw(self):
+        """(raw sums [ny][10], centre [ny][3], count) - additive over slabs when the centre is 0."""
+        raw = np.zeros((self.ny, NSTAT))
+        centre = np.zeros((self.ny, 3))
+        cnt = C.c_double(0.0)
+        _check(lib().lbm_stats_read_raw(self._h, _dp(raw), _dp(centre), C.byref(cnt)))
+        return raw, centre, float(cnt.value)
 
     def set_graphs(self, mode: int):
         """0 off, 1 on, 2 auto (CUDA graphs of ~32 steps inside lbm_step)."""

@@ -73,7 +73,9 @@ struct lbm_s {
     std::vector<double> lad;
     uint32_t bc;
     int bot, top;
-    bool aa, drag_vector, mask;
+    bool aa, drag_vector, mask, halo;
+    int zg0, nzg;               // z slab: global plane of local plane 0, global nz
+    int zlo, zhi;               // planes the step updates: [zlo, zhi)
     std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
     int V, TX, TY, nchunk;
     Layout L;
@@ -166,12 +168,16 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     if (!(nu > 0.0) || !std::isfinite(nu)) return fail(LBM_EINVAL, "nu must be > 0 (got %g)", nu);
     if (!(Cs >= 0.0) || !std::isfinite(Cs)) return fail(LBM_EINVAL, "Cs must be >= 0 (got %g)", Cs);
     if (!(Cd >= 0.0) || !std::isfinite(Cd)) return fail(LBM_EINVAL, "Cd must be >= 0 (got %g)", Cd);
-    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_SOLID_MASK | LBM_STORAGE_AA | LBM_VEC_MASK))
+    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_SOLID_MASK | LBM_STORAGE_AA | LBM_Z_HALO | LBM_VEC_MASK))
         return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
     int bot, top;
     if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
     if ((bc_flags & LBM_SOLID_MASK) && nx % 32)
         return fail(LBM_EINVAL, "LBM_SOLID_MASK needs nx %% 32 == 0 (got nx=%d)", nx);
+    if (bc_flags & LBM_Z_HALO) {
+        if (bc_flags & LBM_STORAGE_AA) return fail(LBM_EINVAL, "LBM_Z_HALO needs two-lattice storage");
+        if (nz < 3) return fail(LBM_EINVAL, "LBM_Z_HALO needs nz >= 3 (two ghost planes + >= 1 interior)");
+    }
     const int V = pick_vec(nx, bc_flags);
     if (V < 0) return fail(LBM_EINVAL, "cells-per-thread override does not divide nx=%d", nx);
     lbm_s *h = new (std::nothrow) lbm_s();
@@ -192,13 +198,18 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->aa = (bc_flags & LBM_STORAGE_AA) != 0;
     h->drag_vector = (bc_flags & LBM_DRAG_VECTOR) != 0;
     h->V = V;
-    if (!pick_shape(nx / V, (long long)ny * nz, 128, &h->TX, &h->TY)) {
+    // (rows of a launch always start at a plane boundary; a slab's interior and its chunked host
+    // transfers are whole planes, so TY must divide ny when the launch does not cover all rows)
+    if (!pick_shape(nx / V, (bc_flags & LBM_Z_HALO) ? (long long)ny : (long long)ny * nz, 128, &h->TX, &h->TY)) {
         delete h;
         return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
     }
     h->nchunk = (nx / V) / h->TX;
     h->mask = (bc_flags & LBM_SOLID_MASK) != 0;
-    h->nfluid.assign(ny, (double)nx * nz);
+    h->halo = (bc_flags & LBM_Z_HALO) != 0;
+    h->zlo = h->halo ? 1 : 0; h->zhi = h->halo ? nz - 1 : nz;
+    h->zg0 = h->halo ? -1 : 0; h->nzg = h->halo ? nz - 2 : nz;
+    h->nfluid.assign(ny, (double)nx * (h->zhi - h->zlo));
     h->L = make_layout(nx, ny, nz, h->aa, h->mask);
     h->ws = nullptr; h->stream = nullptr; h->bound = false; h->inited = false;
     h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
@@ -259,6 +270,7 @@ static void fill_params(lbm_s *h)
     p.partial = nullptr; p.shift = nullptr;
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
     p.z0 = 0; p.z1 = h->nz; p.zoff = 0; p.Nio = h->N;
+    p.zg0 = h->zg0; p.nzg = h->nzg;
 }
 
 int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
@@ -277,6 +289,7 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.partial, 0, h->L.acc - h->L.partial, h->stream));
     if (h->mask) {
         const size_t mbytes = (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4;
         CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, mbytes, h->stream));
@@ -296,14 +309,17 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
     const size_t words = (size_t)nxw * h->ny * h->nz;
     std::vector<uint32_t> bits;
     try { bits.assign(words, 0u); } catch (...) { return fail(LBM_ENOMEM, "host allocation failed"); }
-    h->nfluid.assign(h->ny, (double)h->nx * h->nz);
+    h->nfluid.assign(h->ny, (double)h->nx * (h->zhi - h->zlo));
     if (solid_host)
         for (int z = 0; z < h->nz; ++z)
             for (int y = 0; y < h->ny; ++y) {
                 const uint8_t *row = solid_host + ((size_t)z * h->ny + y) * h->nx;
                 uint32_t *out = bits.data() + ((size_t)z * h->ny + y) * nxw;
                 for (int x = 0; x < h->nx; ++x)
-                    if (row[x]) { out[x >> 5] |= 1u << (x & 31); h->nfluid[y] -= 1.0; }
+                    if (row[x]) {
+                        out[x >> 5] |= 1u << (x & 31);
+                        if (z >= h->zlo && z < h->zhi) h->nfluid[y] -= 1.0;
+                    }
             }
     // the mask dilated by one cell in every direction (periodic x, z; y only where periodic):
     // bit = some cell within one step is solid.  The kernels skip the geometry work where it is 0.
@@ -403,7 +419,7 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
 template <int V, bool S>
 static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
 {
-    dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY * h->nchunk));
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / h->TY * h->nchunk));
     if (h->mask) {
         if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S, true><<<grid, block, 0, h->stream>>>(p);
         else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S, true><<<grid, block, 0, h->stream>>>(p);
@@ -440,7 +456,7 @@ static int stats_reset_impl(lbm_s *h)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
     h->nsamples = 0; h->stats_phase = 0;
-    if (h->inited && !h->mask) {
+    if (h->inited && !h->mask && !h->halo) {
         // centre the accumulation on the current plane means (numerical shift only; not with a
         // solid mask, where the number of contributing cells differs from thread to thread)
         KParams p = h->kp;
@@ -531,9 +547,10 @@ static int step_direct(lbm_s *h, int n)
         const bool sample = h->stats_every > 0 && (h->stats_phase % h->stats_every) == 0;
         KParams p = h->kp;
         if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
+        p.z0 = h->zlo; p.z1 = h->zhi;
         if (sample) {
             p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
-            p.shift = h->mask ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
+            p.shift = (h->mask || h->halo) ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
         }
         const bool timed = h->timing && h->ev_used + 2 <= 2 * MAX_TIMED;
         if (timed) {
@@ -633,6 +650,90 @@ int lbm_step(lbm_t *h, int n)
     return step_direct(h, n);
 }
 
+int lbm_set_z_slab(lbm_t *h, int z_first, int nz_global)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->halo) return fail(LBM_EINVAL, "handle was not created with LBM_Z_HALO");
+    if (nz_global < 1 || z_first < 0 || z_first >= nz_global) return fail(LBM_EINVAL, "bad slab position");
+    h->zg0 = z_first - 1; h->nzg = nz_global;
+    h->kp.zg0 = h->zg0; h->kp.nzg = h->nzg;
+    return LBM_OK;
+}
+
+int lbm_halo_bytes(const lbm_t *h, size_t *bytes)
+{
+    if (!h || !bytes) return fail(LBM_EINVAL, "NULL argument");
+    *bytes = (size_t)5 * h->nx * h->ny * 4;
+    return LBM_OK;
+}
+
+static int halo_copy(lbm_s *h, int side, float *buf, bool pack)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->halo) return fail(LBM_EINVAL, "handle was not created with LBM_Z_HALO");
+    if (!h->inited) return fail(LBM_ESTATE, "halo call before lbm_init / lbm_set_macros");
+    if (!buf || (side != 0 && side != 1)) return fail(LBM_EINVAL, "bad halo arguments");
+    KParams p = h->kp;
+    if (h->t & 1) { float *t = p.src; p.src = p.dst; p.dst = t; }   // the lattice holding state t
+    const long long plane = (long long)h->nx * h->ny;
+    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
+    if (pack) {
+        // leaving data: low face = c_z -1 populations of plane 1, high face = c_z +1 of plane nz-2
+        halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.src, h->N, plane, side ? h->nz - 2 : 1, side, buf);
+    } else {
+        // entering data: through the low face (ghost plane 0) come c_z +1 populations, through the
+        // high face (ghost plane nz-1) c_z -1 populations
+        halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.src, h->N, plane, side ? h->nz - 1 : 0, side ? 0 : 1, buf);
+    }
+    h->launches++;
+    CU_TRY(cudaGetLastError());
+    return LBM_OK;
+}
+
+int lbm_halo_pack(lbm_t *h, int side, float *buf_dev) { return halo_copy(h, side, buf_dev, true); }
+int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev)
+{
+    return halo_copy(h, side, const_cast<float *>(buf_dev), false);
+}
+
+int lbm_stats_read_raw(lbm_t *h, double *out, double *centre, double *count)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_read_raw before lbm_bind");
+    if (!out) return fail(LBM_EINVAL, "out is NULL");
+    std::vector<float> shift((size_t)h->ny * 4);
+    int flag = 0;
+    CU_TRY(cudaMemcpyAsync(out, h->ws + h->L.acc, (size_t)h->ny * NSTAT * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaMemcpyAsync(shift.data(), h->ws + h->L.shift, shift.size() * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaMemcpyAsync(&flag, h->ws + h->L.flag, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    for (int y = 0; y < h->ny; ++y) {
+        out[(size_t)y * NSTAT + 9] += (double)h->nsamples * h->nfluid[y];   // sum of rho, not of rho-1
+        if (centre) for (int a = 0; a < 3; ++a) centre[y * 3 + a] = shift[y * 4 + a];
+    }
+    if (count) *count = (double)h->nsamples * h->nx * (h->zhi - h->zlo);
+    if (flag) return fail(LBM_EDIVERGED, "non-finite plane sum of rho seen by the statistics reduction");
+    return LBM_OK;
+}
+
+int lbm_stats_from_raw(const double *raw, const double *centre, int ny, double count, double *out)
+{
+    if (!raw || !out || ny < 1) return fail(LBM_EINVAL, "bad arguments");
+    for (int y = 0; y < ny; ++y) {
+        const double *a = raw + (size_t)y * NSTAT;
+        double *r = out + (size_t)y * NSTAT;
+        if (!(count > 0.0)) { for (int k = 0; k < NSTAT; ++k) r[k] = 0.0; continue; }
+        const double mu = a[0] / count, mv = a[1] / count, mw = a[2] / count;
+        r[0] = mu + (centre ? centre[y * 3 + 0] : 0.0);
+        r[1] = mv + (centre ? centre[y * 3 + 1] : 0.0);
+        r[2] = mw + (centre ? centre[y * 3 + 2] : 0.0);
+        r[3] = a[3] / count - mu * mu; r[4] = a[4] / count - mv * mv; r[5] = a[5] / count - mw * mw;
+        r[6] = a[6] / count - mu * mv; r[7] = a[7] / count - mv * mw; r[8] = a[8] / count - mu * mw;
+        r[9] = a[9] / count;
+    }
+    return LBM_OK;
+}
+
 int lbm_set_graphs(lbm_t *h, int mode)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
@@ -728,7 +829,7 @@ int lbm_stats_read(lbm_t *h, double *out, long long *nsamples)
     CU_TRY(cudaMemcpyAsync(&flag, h->ws + h->L.flag, 4, cudaMemcpyDeviceToHost, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream));
     if (nsamples) *nsamples = h->nsamples;
-    const double cnt = (double)h->nsamples * h->nx * h->nz;
+    const double cnt = (double)h->nsamples * h->nx * (h->zhi - h->zlo);
     for (int y = 0; y < h->ny; ++y) {
         const double *a = acc.data() + (size_t)y * NSTAT;
         double *r = out + (size_t)y * NSTAT;

@@ -80,7 +80,8 @@ struct KParams {
     const float *uprof;         // [ny] synthetic profile U(y_j)
     double noise_amp;           // noise_frac * U_ref
     unsigned long long seed;
-    int z0, z1;                 // z range for chunked host transfers (macros / set_macros)
+    int z0, z1;                 // z range of a launch (chunked host transfers; interior planes of a slab)
+    int zg0, nzg;               // z slab: global z of local plane 0 and global nz (init recipe only)
     long long zoff;             // element offset of plane z0 inside rho_in/u_in/rho_out/u_out
     long long Nio;              // component stride of u_in / u_out
 };
@@ -707,7 +708,7 @@ template <int V> struct Occ { static constexpr int minb = (V == 4) ? 2 : (V == 2
 template <int V, int RM, int WM, bool STATS, bool MASK = false>
 __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const KParams p)
 {
-    const Ctx c = make_ctx<V>(p, 0);
+    const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
     // With a mask, a warp none of whose lanes has a solid cell within one step (the usual case:
     // geometry is sparse) runs the unmasked load/store code; the decision is warp-uniform, so the
     // full-mask shuffles inside load_dir/store_dir stay converged.
@@ -740,7 +741,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
         }
         collide<V>(p, g, k, m);
     }
-    const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, 0, true) : c;
+    const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
     if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
     else store_all<V, WM, false>(p, c2, g);
     if constexpr (STATS) {
@@ -823,7 +824,10 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const K
             rho = p.rho_in[off + k];
             ux = p.u_in[off + k]; uy = p.u_in[p.Nio + off + k]; uz = p.u_in[2 * p.Nio + off + k];
         } else {
-            const unsigned long long cell = (unsigned long long)(cell0 + k);
+            // global cell index of the recipe (a z slab initialises its part of the global field)
+            int zg = (c.z + p.zg0) % p.nzg;
+            if (zg < 0) zg += p.nzg;
+            const unsigned long long cell = (unsigned long long)((long long)(c.y + p.ny * zg) * p.nx + c.x0 + k);
             const double inv53 = 1.0 / 9007199254740992.0;
             const double r0 = (double)(mix64(p.seed, 3ULL * cell + 0ULL) >> 11) * inv53;
             const double r1 = (double)(mix64(p.seed, 3ULL * cell + 1ULL) >> 11) * inv53;
@@ -926,6 +930,24 @@ __global__ void __launch_bounds__(256) stats_stage2_kernel(const float *__restri
             shift[y * 4 + k] = isfinite(mean) ? (float)mean : 0.f;
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// z-slab halo exchange: the five populations that cross a z face, of one x-y
+// plane, to / from a contiguous buffer [5][ny][nx].  side 1: c_z = +1 (i = 5, 11, 14, 15, 18),
+// side 0: c_z = -1 (i = 6, 12, 13, 16, 17).  pack reads plane `z`, unpack writes plane `z`.
+// ---------------------------------------------------------------------------------------------
+template <bool PACK>
+__global__ void halo_kernel(float *pops, long long N, long long plane, int z, int side, float *buf)
+{
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= 5 * plane) return;
+    const int j = (int)(q / plane);
+    const long long r = q - (long long)j * plane;
+    const int up[5] = {5, 11, 14, 15, 18}, dn[5] = {6, 12, 13, 16, 17};
+    const int i = side ? up[j] : dn[j];
+    float *cell = pops + (long long)i * N + (long long)z * plane + r;
+    if (PACK) buf[q] = *cell; else *cell = buf[q];
 }
 
 } // namespace lbm

@@ -1,0 +1,161 @@
+"""z-slab decomposition.
+
+GPU: all ranks of a ring emulated one after another on one GPU must reproduce the undivided
+lattice bit for bit (same kernels, same arithmetic per cell).  CPU: the ring exchange and the
+statistics reduction over torch.distributed with gloo, world sizes 2 and 3."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU: ring exchange over gloo
+# ---------------------------------------------------------------------------------------------
+def _ring_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+
+    sys.path.insert(0, ROOT)
+    from paper_2206_15454_b200.slab import ring_exchange, ring_neighbours
+
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    hi = torch.full((5, 3, 4), rank * 10.0 + 1.0)
+    lo = torch.full((5, 3, 4), rank * 10.0 + 2.0)
+    from_lower, from_upper = torch.zeros(5, 3, 4), torch.zeros(5, 3, 4)
+    for _ in range(3):                                   # repeated exchanges stay paired
+        ring_exchange(hi, lo, from_lower, from_upper, rank, world)
+    lower, upper = ring_neighbours(rank, world)
+    ok = bool((from_lower == lower * 10.0 + 1.0).all() and (from_upper == upper * 10.0 + 2.0).all())
+    t = torch.tensor([float(rank + 1)], dtype=torch.float64)
+    dist.all_reduce(t)
+    q.put((rank, ok, float(t)))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_ring_exchange_gloo(world):
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_ring_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = [q.get(timeout=180) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _ in got)
+    assert all(s == world * (world + 1) / 2 for _, _, s in got)
+
+
+def test_ring_exchange_single_rank_is_self_periodic():
+    import torch
+    from paper_2206_15454_b200.slab import ring_exchange, ring_neighbours
+
+    hi, lo = torch.ones(2, 2), 2 * torch.ones(2, 2)
+    a, b = torch.zeros(2, 2), torch.zeros(2, 2)
+    ring_exchange(hi, lo, a, b, 0, 1)
+    assert (a == 1).all() and (b == 2).all()
+    assert ring_neighbours(0, 4) == (3, 1) and ring_neighbours(3, 4) == (2, 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# GPU: emulated ring == undivided lattice
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 2, 3, 4])
+@pytest.mark.parametrize("case", ["forest", "lid+solid"])
+def test_emulated_slabs_equal_global_lattice(world, case):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    cfg = wl.small(nx=32, ny=10, nz=12)
+    if case == "lid+solid":
+        cfg = wl.small(nx=32, ny=10, nz=12, top=wl.FORCED_EQ)
+        cfg["U_top"] = (0.06, 0.0, 0.01)
+        m = np.zeros((12, 10, 32), bool)
+        m[0:2, 0:3, 4:9] = True                          # a box that straddles the z wrap ...
+        m[11, 0:3, 4:9] = True
+        m[5:7, 2:5, 30:] = True                          # ... and one across a slab face and the x wrap
+        m[5:7, 2:5, :2] = True
+        cfg["solid"] = m
+    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref.init(cfg["seed"])
+    ref.stats_accumulate(1)
+    ref.stats_reset()
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True) for r in range(world)]
+    slab.init_emulated(slabs, cfg["seed"])
+    for s in slabs:
+        s.stats_accumulate(1)
+        s.stats_reset()
+    for n in (1, 2, 6):
+        ref.step(n)
+        slab.step_emulated(slabs, n)
+        rr, ur = ref.get_macros()
+        rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
+        us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
+        assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
+    sr, nr = ref.stats_read()
+    ss = slab.stats_emulated(slabs)
+    assert nr == 9
+    # the undivided run centres its fp32 row sums, the slabs do not: equal to fp32 summation noise
+    assert np.abs(ss[:, 0:3] - sr[:, 0:3]).max() <= 1e-6 * cfg["u_bulk"]
+    assert np.abs(ss[:, 3:9] - sr[:, 3:9]).max() <= 1e-6 * cfg["u_bulk"] ** 2
+    assert np.abs(ss[:, 9] - sr[:, 9]).max() <= 1e-7
+    for s in slabs:
+        s.close()
+
+
+@pytest.mark.gpu
+def test_single_slab_through_torch_distributed_path():
+    """world == 1 through SlabLbm.step itself (self-periodic exchange) == undivided lattice."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    cfg = wl.small(nx=64, ny=8, nz=6)
+    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref.init(3)
+    s = slab.SlabLbm(cfg, 0, 1)
+    s.init(3)
+    s.stats_accumulate(2)
+    ref.step(5)
+    s.step(5)
+    assert torch.equal(s.get_macros()[1], ref.get_macros()[1])
+    st = s.stats_read()
+    assert np.isfinite(st).all() and abs(st[:, 9].mean() - 1.0) < 1e-6
+
+
+@pytest.mark.gpu
+def test_halo_flag_rules():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    with pytest.raises(lb.LbmError):                      # AA storage pushes into the ghost planes
+        lb.Lbm(32, 4, 6, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip", aa=True, halo=True))
+    with pytest.raises(lb.LbmError):
+        lb.Lbm(32, 4, 2, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip", halo=True))
+    g = lb.Lbm(32, 4, 6, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip"))
+    with pytest.raises(lb.LbmError):
+        g.set_z_slab(0, 4)
