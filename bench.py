@@ -352,6 +352,70 @@ def run_b200(args, cfg):
     return 0
 
 
+def run_sharded(args, cfg):
+    """--sharded: ONE lattice of nx x ny x (N nz) cut into N z slabs (two-lattice storage), one
+    halo exchange per step over torch.distributed.  Opt-in: the default --gpus N
+    path stays N replicas, because this run's hardware has one GPU and the NCCL leg could only be
+    exercised with N = 1 (self exchange) and emulated rings."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    g = dict(cfg)
+    g["nz"] = cfg["nz"] * world
+    g["storage"] = "two_lattice"
+    K, W = args.steps, args.warmup
+    N = wl.n_cells(cfg)
+    s = slab.SlabLbm(g, rank, world, device=dev)
+    s.init(cfg["seed"])
+    s.stats_accumulate(cfg.get("stats_every", 0))
+    s.step(W)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.begin()
+    stream = torch.cuda.current_stream(dev)
+    l0 = s.sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    s.step(K)
+    e1.record(stream)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms = max_over_ranks([e0.elapsed_time(e1)], world, dev)[0]
+    launches = s.sim.launch_count - l0
+    clocks = sampler.result()
+    st = s.stats_read()
+    if not np.isfinite(st).all():
+        raise RuntimeError("sharded run produced non-finite statistics")
+    if rank == 0:
+        mlups = aggregate_mlups(N, K, ms, world)
+        cfgd = workload_config(g, args, s.sim.variant)
+        cfgd["parallelism"] = f"one lattice in {world} z slab(s), ring halo exchange of 2 x 5 x nx x ny fp32 per step"
+        print(json.dumps({
+            "metric": METRIC, "value": round(mlups, 1), "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": W, "ms_per_step": round(ms / K, 5), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfgd,
+            "algorithmic_gbs": round(mlups * BYTES_PER_CELL / 1e3 / world, 1),
+            "halo_bytes_per_step": 2 * 5 * cfg["nx"] * cfg["ny"] * 4,
+            "gpu_launches": int(launches), "clocks": clocks, "mode": "sharded"}))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -366,6 +430,8 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes (read+write) per step-kernel launch, from profiles/, to quote in the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sharded", action="store_true",
+                    help="one lattice cut into N z slabs with a halo exchange per step (opt-in)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -376,6 +442,8 @@ def main():
         cfg["stats_every"] = args.stats_every
     if args.impl == "reference":
         return run_reference(args, cfg)
+    if args.sharded:
+        return run_sharded(args, cfg)
     return run_b200(args, cfg)
 
 
