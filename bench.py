@@ -38,9 +38,10 @@ import workloads as wl  # noqa: E402
 
 BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star)
 # dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch / cells, from the one
-# `ncu --set full` capture of the current kernel (profiles/r01_README.md: cfg4, both AA parities
-# 151.7 B/cell).  The bench line scales it by the cell count of the timed workload and says so.
-NCU_TRAFFIC_BYTES_PER_CELL = {"aa": 151.7}
+# `ncu --set full` captures of the current kernels (profiles/r01_README.md: AA, cfg4, both
+# parities 151.7 B/cell; two-lattice pull, cfg3, 149.0 B/cell - part of its last writes is still
+# in L2 when the launch ends).  The bench line scales it by the cell count and says so.
+NCU_TRAFFIC_BYTES_PER_CELL = {"aa": 151.7, "two_lattice": 149.0}
 METRIC = "MLUPS"
 UNIT = "MLUPS (1e6 lattice-cell updates/s)"
 
@@ -318,7 +319,7 @@ def run_b200(args, cfg):
         traffic, traffic_src = args.traffic, "command line (--traffic)"
         if traffic is None and cfg["storage"] in NCU_TRAFFIC_BYTES_PER_CELL:
             traffic = round(NCU_TRAFFIC_BYTES_PER_CELL[cfg["storage"]] * N)
-            traffic_src = ("ncu --set full on cfg4 (profiles/r01_README.md): "
+            traffic_src = ("ncu --set full (profiles/r01_README.md: AA on cfg4, two-lattice on cfg3): "
                            f"{NCU_TRAFFIC_BYTES_PER_CELL[cfg['storage']]} B/cell x {N} cells")
         elif traffic is None:
             traffic_src = None
