@@ -605,3 +605,65 @@ def test_p15_mass_conserved_with_solids(orc):
     o.step(300)
     m1 = o.get_populations()[:, ~solid].sum()
     assert abs(m1 - m0) <= 1e-12 * m0
+
+
+# ------------------------------------------------------------------------------------------
+# P16: the Pi_neq assembly INSIDE the collision (oracle step O7 -> O8 -> O9)
+# ------------------------------------------------------------------------------------------
+
+def _p16_state(w, c, rho, u, A):
+    """f_i = f_eq,i(rho, u) + w_i (9/2) (c_i c_i - I/3) : A  for a symmetric traceless A.
+    The added part has zero mass and momentum (sum w = 1, sum w c c = I/3, odd moments vanish)
+    and second moment exactly A (fourth-order isotropy, pinned by P0), so Pi_neq = A."""
+    cu = c @ u
+    feq = w * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u @ u))       # Eq. 3 (L52), typed here
+    Qi = np.einsum("ia,ib->iab", c, c) - np.eye(3) / 3
+    fneq = w * 4.5 * np.einsum("iab,ab->i", Qi, A)
+    return feq, fneq
+
+
+@pytest.mark.parametrize("Cs", [0.1, 0.17, 0.0])
+def test_p16_relaxation_of_a_known_pi_neq(orc, Cs):
+    """PAPER.md:L69 (Pi = Pi_eq + Pi_neq), L87 Eq. 11 (Q^1/2 = sqrt(Pi_neq : Pi_neq)), L91-94
+    (tau_total replaces tau in Eq. 2), as used inside the collision.  On a periodic, spatially
+    uniform state streaming is the identity; with F = 0 one step must give
+        f*_i - f_eq,i = (1 - 1/tau_t) f_neq,i,   tau_t = (tau0 + sqrt(tau0^2 + 18 sqrt2 Cs^2 sqrt(A:A)/rho))/2
+    with rho, u unchanged.  A dropped rho, a missing rho u u term, a transposed or halved
+    off-diagonal in the Pi_neq assembly all change Q and hence tau_t."""
+    c, w, _, _ = orc.tables()
+    c = c.astype(float)
+    rng = np.random.default_rng(16)
+    nx, ny, nz = 4, 3, 5
+    for trial in range(12):
+        B = rng.normal(size=(3, 3))
+        A = 0.5 * (B + B.T)
+        A -= np.trace(A) / 3 * np.eye(3)
+        A *= 10 ** rng.uniform(-4, -2.3)
+        rho = rng.uniform(0.9, 1.1)
+        u = rng.uniform(-0.12, 0.12, 3)
+        if trial == 0:
+            u = np.array([0.1, -0.07, 0.05])          # never a near-zero velocity on the first case
+        nu = 10 ** rng.uniform(-4, -2)
+        tau0 = 3 * nu + 0.5
+        feq, fneq = _p16_state(w, c, rho, u, A)
+        # the construction itself: mass, momentum and second moment of the added part
+        assert abs(fneq.sum()) < 1e-17 and np.abs(fneq @ c).max() < 1e-17
+        assert np.allclose(np.einsum("i,ia,ib->ab", fneq, c, c), A, rtol=0, atol=1e-17)
+        o = orc.Oracle(nx, ny, nz, nu, Cs, (0, 0, 0), 0.0, None, _periodic_bc(orc))
+        o.set_populations(np.broadcast_to((feq + fneq)[:, None, None, None], (19, nz, ny, nx)).copy())
+        r0, u0 = o.get_macros()
+        assert np.abs(r0 - rho).max() < 1e-15 and np.abs(u0 - u[:, None, None, None]).max() < 1e-15
+        o.step(1)
+        fs = o.get_populations()
+        Qh = np.sqrt(np.sum(A * A))
+        tau_t = 0.5 * (tau0 + np.sqrt(tau0 ** 2 + 18 * np.sqrt(2) * Cs ** 2 * Qh / rho))
+        want = feq + (1 - 1 / tau_t) * fneq
+        got = fs[:, 2, 1, 3]
+        assert np.abs(fs - got[:, None, None, None]).max() < 1e-16        # still uniform
+        # a few ulp of the O(1/3) populations; a slip in the Pi_neq assembly moves tau_t and
+        # shows at |delta(1/tau)| * |f_neq| ~ 1e-9 .. 1e-6
+        assert np.abs(got - want).max() <= 1e-15
+        if Cs > 0:
+            # the pin has teeth: tau0 instead of tau_t would miss by far more than the bound
+            miss = np.abs((1 / tau0 - 1 / tau_t) * fneq).max()
+            assert miss > 1e-6 * np.abs(fneq).max() > 1e-11
