@@ -17,8 +17,9 @@ One JSON line is printed by rank 0:
                (CUDA events recorded by the library on its launch stream, lbm_set_kernel_timing)
                against MEASURED_PEAKS.json's hbm_gbs
   cpu_baseline the fp64 oracle, as it stands, on the host cores on a bounded slab of the workload
---gpus N > 1: the path is built for one GPU (replicas only); every rank
-runs an independent replica of the workload and `value` is the sum over replicas.
+--gpus N > 1: north_star asks for one GPU; by default every rank runs an independent replica of
+the workload and `value` is the sum over replicas.  --sharded instead cuts ONE lattice of
+nx x ny x (N nz) cells into N z slabs with a halo exchange per step.
 --impl reference times the oracle alone (the reference arm of this tier).
 """
 from __future__ import annotations
@@ -37,11 +38,13 @@ if ROOT not in sys.path:
 import workloads as wl  # noqa: E402
 
 BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star)
-# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch / cells, from the one
-# `ncu --set full` captures of the current kernels (profiles/r01_README.md: AA, cfg4, both
-# parities 151.7 B/cell; two-lattice pull, cfg3, 149.0 B/cell - part of its last writes is still
-# in L2 when the launch ends).  The bench line scales it by the cell count and says so.
-NCU_TRAFFIC_BYTES_PER_CELL = {"aa": 151.7, "two_lattice": 149.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch / cells, from ncu captures
+# of the current kernels on the named config (profiles/): the line quotes the figure of its own
+# config when one exists, else null.
+NCU_TRAFFIC_BYTES_PER_CELL = {
+    ("cfg4", "aa"): (151.7, "profiles/r01_README.md, ncu --set full on cfg4, both AA parities"),
+    ("cfg3", "two_lattice"): (149.0, "profiles/r01_README.md, ncu --set full on cfg3"),
+}
 METRIC = "MLUPS"
 UNIT = "MLUPS (1e6 lattice-cell updates/s)"
 
@@ -170,12 +173,21 @@ def run_reference(args, cfg):
     steps = args.steps
     # bounded sample: each step is one oracle time step of a 128 x ny x 32 slab (~0.3 s)
     mlups, ms, steps_done, cores, sample = time_oracle(cfg, steps, args.warmup, max_nx=128, max_nz=32)
+    ran = oracle_sample_config(cfg, 128, 32)
+    conf = workload_config(cfg, args, None)
+    # the lattice the oracle actually advanced (a bounded x-z sub-slab of the workload, full ny)
+    conf["lattice"] = [ran["nx"], ran["ny"], ran["nz"]]
+    conf["cells"] = wl.n_cells(ran)
+    conf["full_workload_lattice"] = [cfg["nx"], cfg["ny"], cfg["nz"]]
+    conf["storage"] = "two_lattice fp64 (oracle)"
+    conf["l2"] = "oracle on host cores; no GPU cache involved"
+    conf["parallelism"] = f"{cores} host threads (OpenMP)"
     line = {
         "impl": "reference", "metric": METRIC, "value": round(mlups, 3), "unit": UNIT,
         "n_gpus": args.gpus, "steps": steps_done, "warmup": args.warmup,
         "ms_per_step": round(ms, 4), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, args, None),
+        "config": conf,
         "cpu_baseline": {"value": round(mlups, 3), "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": round(mlups, 3), "unit": UNIT, "h2d_bytes_per_step": 0,
@@ -259,12 +271,22 @@ def run_b200(args, cfg):
     stream = torch.cuda.current_stream(dev)
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps ----
+    # roofline leg: the step kernel alone, each launch bracketed by a pair of CUDA events that the
+    # library records on its launch stream.  On lattices whose step takes milliseconds the
+    # brackets sit INSIDE the K timed steps (the same launches give `value` and
+    # `roofline.achieved`, so kernel_ms <= ms_per_step by construction; two event records per
+    # >= 3 ms step cost nothing measurable).  Smaller lattices are timed without brackets (a pair
+    # of event records is comparable to their launch gaps, and lbm_step replays CUDA graphs
+    # there) and bracketed in a second K-step pass.
+    same_pass = N * BYTES_PER_CELL / 6.5e12 > 1e-3 and K <= 4096
     sim.step(W)
     barrier()
     sampler = ClockSampler(local)
     sampler.begin()
     l0 = sim.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if same_pass:
+        sim.set_kernel_timing(True)
     e0.record(stream)
     sim.step(K)
     e1.record(stream)
@@ -275,11 +297,9 @@ def run_b200(args, cfg):
     stats, nsamp = sim.stats_read()
     if every > 0 and (nsamp != (W + K) // every or not np.isfinite(stats).all()):
         raise RuntimeError(f"statistics check failed: nsamples={nsamp}, finite={np.isfinite(stats).all()}")
-
-    # ---- roofline leg: the step kernel alone, bracketed per launch by the library ----
-    sim.set_kernel_timing(True)
-    nk = min(K, 4096)
-    sim.step(nk)
+    if not same_pass:
+        sim.set_kernel_timing(True)
+        sim.step(min(K, 4096))
     k_ms, k_n = sim.kernel_timing_read()
     sim.set_kernel_timing(False)
     kernel_ms = k_ms / max(1, k_n)
@@ -317,10 +337,11 @@ def run_b200(args, cfg):
         e2e_mlups = aggregate_mlups(N, e2e_steps, e2e_ms, world)
         achieved = BYTES_PER_CELL * N / (kernel_ms * 1e-3) / 1e9
         traffic, traffic_src = args.traffic, "command line (--traffic)"
-        if traffic is None and cfg["storage"] in NCU_TRAFFIC_BYTES_PER_CELL:
-            traffic = round(NCU_TRAFFIC_BYTES_PER_CELL[cfg["storage"]] * N)
-            traffic_src = ("ncu --set full (profiles/r01_README.md: AA on cfg4, two-lattice on cfg3): "
-                           f"{NCU_TRAFFIC_BYTES_PER_CELL[cfg['storage']]} B/cell x {N} cells")
+        key = (cfg["name"], cfg["storage"])
+        if traffic is None and key in NCU_TRAFFIC_BYTES_PER_CELL:
+            bpc, where = NCU_TRAFFIC_BYTES_PER_CELL[key]
+            traffic = round(bpc * N)
+            traffic_src = f"{where}: {bpc} B/cell x {N} cells"
         elif traffic is None:
             traffic_src = None
         line = {
@@ -335,7 +356,9 @@ def run_b200(args, cfg):
                          "frac": round(achieved / peak, 4), "traffic": traffic,
                          "traffic_source": traffic_src,
                          "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL,
-                         "kernel_ms": round(kernel_ms, 5), "launches_timed": k_n},
+                         "kernel_ms": round(kernel_ms, 5), "launches_timed": k_n,
+                         "timed_in": "the K timed steps themselves" if same_pass else
+                                     "a second K-step pass (the timed pass runs unbracketed)"},
             "e2e": {"value": round(e2e_mlups, 1), "unit": UNIT,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps,
@@ -420,7 +443,9 @@ def run_sharded(args, cfg):
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed steps; default: the count BASELINE.json states for the config "
+                         "(cfg5: 500, cfg4: 1000), 200 for the small ones")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 (BASELINE.json:configs[0..4])")
@@ -437,6 +462,11 @@ def main():
     if args.warmup < 3:
         args.warmup = 3
     cfg = wl.get(args.config)
+    if args.steps is None:
+        # BASELINE.json:configs[3,4] state the timed step counts (1000, 500); the reference arm's
+        # steps are oracle steps on a bounded slab (~0.3 s each), kept to a few minutes
+        args.steps = 20 if args.impl == "reference" else (
+            cfg["steps"] if cfg["name"] in ("cfg4", "cfg5") else 200)
     if args.storage:
         cfg["storage"] = args.storage
     if args.stats_every is not None:

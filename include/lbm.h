@@ -20,7 +20,9 @@
  *     library never allocates population memory: the caller (the Python binding uses
  *     torch.empty) owns one device workspace of lbm_workspace_bytes() bytes, 256-byte aligned,
  *     and must keep it alive until lbm_destroy.  All kernels are launched on the CUDA stream
- *     given to lbm_bind (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *     given to lbm_bind (a cudaStream_t passed as void*; NULL = legacy default stream), which
+ *     must belong to the device that holds the workspace.  lbm_bind records that device and every
+ *     later call runs under it (the caller's current device is restored on return).
  *   - All calls on one handle must come from one host thread at a time.
  *   - Time: "state k" is the post-collision population set after k steps.  The sample
  *     S_k = (rho, u) is obtained by streaming state k and applying Eqs. 5-6 and 13 (what step
@@ -179,11 +181,25 @@ int lbm_stats_accumulate(lbm_t *h, int every);
 int lbm_stats_read(lbm_t *h, double *out_host, long long *nsamples);
 int lbm_stats_reset(lbm_t *h);
 
-/* Raw copy of the population array(s) in the library's internal representation, for
- * checkpointing and tests: device [19][nz][ny][nx] fp32 of f_i - w_i in SPECIFICATION numbering
- * (include/lbm.h velocity table below), converted to the plain "state k" (post-collision,
- * un-streamed) representation whatever the storage mode/parity. */
+/* Checkpoint / restart and tests: the populations in the plain "state k" representation
+ * (post-collision, un-streamed), device [19][nz][ny][nx] fp32 of f_i - w_i in SPECIFICATION
+ * numbering (velocity table below), whatever the storage mode and time parity hold internally.
+ * lbm_get_state writes it (state unchanged).  lbm_set_state installs it as state t (t >= 0: the
+ * step counter the state belongs to; its parity selects the AA representation / the lattice of
+ * the two-lattice scheme), so that get_state -> set_state(., lbm_time) -> lbm_step continues a
+ * run bit for bit, non-equilibrium part included (lbm_set_macros would discard it).  Solid cells
+ * are stored as the rest state.  The statistics sums and the sampling phase are left as they are.
+ * Both are asynchronous on the bound stream.  lbm_set_state: LBM_ESTATE before lbm_bind. */
 int lbm_get_state(lbm_t *h, float *f_minus_w_dev);
+int lbm_set_state(lbm_t *h, const float *f_minus_w_dev, long long t);
+
+/* Divergence sentinel: the stage-2 statistics reduction and lbm_get_macros* set a
+ * device flag when they meet a non-finite density.  lbm_stats_read, lbm_stats_read_raw and
+ * lbm_get_macros_host return LBM_EDIVERGED once it is set; lbm_get_macros is asynchronous, so its
+ * finding is reported by the next of those calls or by lbm_diverged, which synchronises the stream,
+ * writes the flag (0/1) to *flag_host (may be NULL) and returns LBM_OK or LBM_EDIVERGED.  The flag
+ * is cleared by lbm_init, lbm_set_macros* and lbm_stats_reset. */
+int lbm_diverged(lbm_t *h, int *flag_host);
 
 /* Number of steps taken since the last init / set_macros. */
 long long lbm_time(const lbm_t *h);
@@ -192,8 +208,10 @@ long long lbm_time(const lbm_t *h);
 long long lbm_launch_count(const lbm_t *h);
 
 /* Tuning hook: override the thread-block shape (tx thread columns of V cells along x, ty rows;
- * tx*ty <= 256, tx divides nx/V with at most 8 blocks per row, ty divides ny*nz).  Call before
- * the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
+ * tx*ty <= 256, tx divides nx/V with at most 8 blocks per row, ty divides ny*nz - or ny itself on
+ * a handle that launches plane ranges: LBM_Z_HALO, or a lattice larger than the host-transfer
+ * staging area, 256 MB unless the environment variable LBM_STAGING_BYTES says otherwise).  Call
+ * before the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
 
 /* Measurement hook (bench.py "roofline"): with on != 0, lbm_step brackets every step-kernel

@@ -41,6 +41,7 @@ SYMBOLS = [
     "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
+    "lbm_set_state", "lbm_diverged",
 ]
 
 
@@ -88,6 +89,8 @@ def lib():
         L.lbm_stats_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.lbm_stats_reset.argtypes = [vp]
         L.lbm_get_state.argtypes = [vp, fp]
+        L.lbm_set_state.argtypes = [vp, fp, C.c_longlong]
+        L.lbm_diverged.argtypes = [vp, C.POINTER(C.c_int)]
         L.lbm_time.argtypes = [vp]
         L.lbm_time.restype = C.c_longlong
         L.lbm_launch_count.argtypes = [vp]
@@ -349,6 +352,18 @@ class Lbm:
         out = torch.empty((19,) + self.shape, dtype=torch.float32, device=self.device)
         _check(lib().lbm_get_state(self._h, C.c_void_p(out.data_ptr())))
         return out
+
+    def set_state(self, f_minus_w, t: int = 0):
+        """Install a (19, nz, ny, nx) CUDA tensor of f_i - w_i as the plain state of step t."""
+        _check(lib().lbm_set_state(self._h, self._dev(f_minus_w, (19,) + self.shape), int(t)))
+
+    def diverged(self) -> bool:
+        """True once lbm_get_macros* or the statistics reduction has seen a non-finite density."""
+        flag = C.c_int(0)
+        rc = lib().lbm_diverged(self._h, C.byref(flag))
+        if rc not in (LBM_OK, LBM_EDIVERGED):
+            _check(rc)
+        return bool(flag.value)
 
     def stats_accumulate(self, every: int = 1):
         _check(lib().lbm_stats_accumulate(self._h, int(every)))

@@ -36,6 +36,18 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 constexpr int MAX_NCHUNK = 8;
 constexpr size_t STAGING_BUDGET = (size_t)256 << 20;
 
+// Size of the host-transfer staging area.  LBM_STAGING_BYTES (environment, read at every call)
+// overrides the 256 MB default so that tests can force chunked transfers on small lattices.
+static size_t staging_budget()
+{
+    const char *e = getenv("LBM_STAGING_BYTES");
+    if (e && *e) {
+        const long long v = atoll(e);
+        if (v > 0) return (size_t)v;
+    }
+    return STAGING_BUDGET;
+}
+
 struct Layout {
     size_t pops, pops2, partial, acc, shift, cda, uprof, flag, solid, solid_nb, staging, total;
     int stage_planes;
@@ -57,7 +69,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     L.solid_nb = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     const size_t plane = (size_t)16 * nx * ny;
-    size_t planes = STAGING_BUDGET / plane;
+    size_t planes = staging_budget() / plane;
     if (planes < 1) planes = 1;
     if (planes > (size_t)nz) planes = nz;
     L.stage_planes = (int)planes;
@@ -74,6 +86,7 @@ struct lbm_s {
     uint32_t bc;
     int bot, top;
     bool aa, drag_vector, mask, halo;
+    bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
     int zg0, nzg;               // z slab: global plane of local plane 0, global nz
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
     std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
@@ -81,6 +94,7 @@ struct lbm_s {
     Layout L;
     char *ws;
     cudaStream_t stream;
+    int device;                 // CUDA device ordinal of the workspace (-1 before lbm_bind)
     bool bound, inited;
     long long t;
     int stats_every;
@@ -100,6 +114,19 @@ struct lbm_s {
     size_t ev_used;
 };
 constexpr size_t MAX_TIMED = 4096;
+
+// Every entry point that touches the device runs under the device that owns the workspace
+// (recorded at lbm_bind), whatever device is current in the calling thread.
+struct DevGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DevGuard(const lbm_s *h)
+    {
+        if (h && h->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != h->device)
+            switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 static void graph_drop(lbm_s *h)
 {
@@ -198,20 +225,22 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->aa = (bc_flags & LBM_STORAGE_AA) != 0;
     h->drag_vector = (bc_flags & LBM_DRAG_VECTOR) != 0;
     h->V = V;
-    // (rows of a launch always start at a plane boundary; a slab's interior and its chunked host
-    // transfers are whole planes, so TY must divide ny when the launch does not cover all rows)
-    if (!pick_shape(nx / V, (bc_flags & LBM_Z_HALO) ? (long long)ny : (long long)ny * nz, 128, &h->TX, &h->TY)) {
+    h->mask = (bc_flags & LBM_SOLID_MASK) != 0;
+    h->halo = (bc_flags & LBM_Z_HALO) != 0;
+    h->L = make_layout(nx, ny, nz, h->aa, h->mask);
+    // Rows of a launch always start at a plane boundary.  A launch that covers only some planes
+    // (a slab's interior; the chunked host transfers when the staging area holds fewer than nz
+    // planes) has planes*ny rows, so TY must divide ny there; otherwise TY | ny*nz is enough.
+    h->partial_launches = h->halo || h->L.stage_planes < nz;
+    if (!pick_shape(nx / V, h->partial_launches ? (long long)ny : (long long)ny * nz, 128, &h->TX, &h->TY)) {
         delete h;
         return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
     }
     h->nchunk = (nx / V) / h->TX;
-    h->mask = (bc_flags & LBM_SOLID_MASK) != 0;
-    h->halo = (bc_flags & LBM_Z_HALO) != 0;
     h->zlo = h->halo ? 1 : 0; h->zhi = h->halo ? nz - 1 : nz;
     h->zg0 = h->halo ? -1 : 0; h->nzg = h->halo ? nz - 2 : nz;
     h->nfluid.assign(ny, (double)nx * (h->zhi - h->zlo));
-    h->L = make_layout(nx, ny, nz, h->aa, h->mask);
-    h->ws = nullptr; h->stream = nullptr; h->bound = false; h->inited = false;
+    h->ws = nullptr; h->stream = nullptr; h->device = -1; h->bound = false; h->inited = false;
     h->t = 0; h->stats_every = 0; h->stats_phase = 0; h->nsamples = 0; h->launches = 0;
     h->init_kind = LBM_INIT_REST; h->U_ref = 0.0; h->noise_frac = 0.0;
     h->timing = false; h->ev_used = 0;
@@ -226,11 +255,12 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     const int W = h->nx / h->V;
-    if (tx < 1 || ty < 1 || tx * ty > MAX_THREADS || W % tx || (W / tx) > MAX_NCHUNK ||
-        ((long long)h->ny * h->nz) % ty)
-        return fail(LBM_EINVAL, "launch shape %dx%d does not tile %d thread columns x %lld rows", tx, ty, W,
-                    (long long)h->ny * h->nz);
+    const long long rows = h->partial_launches ? (long long)h->ny : (long long)h->ny * h->nz;
+    if (tx < 1 || ty < 1 || tx * ty > MAX_THREADS || W % tx || (W / tx) > MAX_NCHUNK || rows % ty)
+        return fail(LBM_EINVAL, "launch shape %dx%d does not tile %d thread columns x %lld rows%s", tx, ty, W,
+                    rows, h->partial_launches ? " (ty must divide ny: this handle launches plane ranges)" : "");
     graph_drop(h);
     h->TX = tx; h->TY = ty; h->nchunk = W / tx;
     h->kp.nchunk = h->nchunk;
@@ -249,8 +279,6 @@ static void fill_params(lbm_s *h)
     p.tau0 = (float)tau0; p.tau0sq = (float)(tau0 * tau0);
     p.ksmag = (float)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs); // R9: C_smag = Cs^2
     p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
-    // the fp64 momentum channel adds the same (fp32-rounded) force the fp32 terms use
-    p.Fb64[0] = (double)p.Fbx; p.Fb64[1] = (double)p.Fby; p.Fb64[2] = (double)p.Fbz;
     p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
     {
@@ -268,6 +296,7 @@ static void fill_params(lbm_s *h)
     p.solid_nb = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid_nb) : nullptr;
     p.nxw = (h->nx + 31) / 32;
     p.partial = nullptr; p.shift = nullptr;
+    p.diverged = reinterpret_cast<int *>(h->ws + h->L.flag);
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
     p.z0 = 0; p.z1 = h->nz; p.zoff = 0; p.Nio = h->N;
     p.zg0 = h->zg0; p.nzg = h->nzg;
@@ -279,6 +308,14 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     if (!dev_workspace) return fail(LBM_EINVAL, "workspace is NULL");
     if (bytes < h->L.total) return fail(LBM_ENOMEM, "workspace too small: %zu < %zu bytes", bytes, h->L.total);
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) return fail(LBM_ENOMEM, "workspace must be 256-byte aligned");
+    {
+        cudaPointerAttributes at;
+        CU_TRY(cudaPointerGetAttributes(&at, dev_workspace));
+        if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+            return fail(LBM_EINVAL, "workspace is not device memory");
+        h->device = at.device;
+    }
+    DevGuard dg(h);
     graph_drop(h);
     h->ws = static_cast<char *>(dev_workspace);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -303,6 +340,7 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
 int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->mask) return fail(LBM_EINVAL, "handle was not created with LBM_SOLID_MASK");
     if (!h->bound) return fail(LBM_ESTATE, "lbm_set_solid before lbm_bind");
     const int nxw = (h->nx + 31) / 32;
@@ -351,6 +389,7 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
 int lbm_set_top_velocity(lbm_t *h, const double *U_top)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!U_top) return fail(LBM_EINVAL, "U_top is NULL");
     if (h->top != BC_TOP_LID) return fail(LBM_EINVAL, "handle was not created with LBM_TOP_FORCED_EQ");
     for (int a = 0; a < 3; ++a)
@@ -486,6 +525,7 @@ static int upload_profile(lbm_s *h)
 int lbm_init(lbm_t *h, uint64_t seed)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_init before lbm_bind");
     int rc = upload_profile(h);
     if (rc) return rc;
@@ -503,6 +543,7 @@ int lbm_init(lbm_t *h, uint64_t seed)
 int lbm_set_macros(lbm_t *h, const float *rho_dev, const float *u_dev)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_set_macros before lbm_bind");
     if (!rho_dev || !u_dev) return fail(LBM_EINVAL, "rho / u is NULL");
     fill_params(h);
@@ -516,6 +557,7 @@ int lbm_set_macros(lbm_t *h, const float *rho_dev, const float *u_dev)
 int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_set_macros_host before lbm_bind");
     if (!rho_host || !u_host) return fail(LBM_EINVAL, "rho / u is NULL");
     fill_params(h);
@@ -623,6 +665,7 @@ static int graph_build(lbm_s *h, int G)
 int lbm_step(lbm_t *h, int n)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init / lbm_set_macros");
     if (n < 0) return fail(LBM_EINVAL, "n must be >= 0");
     // small lattices are launch-bound: replay G steps as one CUDA graph (identical kernels and
@@ -670,6 +713,7 @@ int lbm_halo_bytes(const lbm_t *h, size_t *bytes)
 static int halo_copy(lbm_s *h, int side, float *buf, bool pack)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->halo) return fail(LBM_EINVAL, "handle was not created with LBM_Z_HALO");
     if (!h->inited) return fail(LBM_ESTATE, "halo call before lbm_init / lbm_set_macros");
     if (!buf || (side != 0 && side != 1)) return fail(LBM_EINVAL, "bad halo arguments");
@@ -699,6 +743,7 @@ int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev)
 int lbm_stats_read_raw(lbm_t *h, double *out, double *centre, double *count)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_read_raw before lbm_bind");
     if (!out) return fail(LBM_EINVAL, "out is NULL");
     std::vector<float> shift((size_t)h->ny * 4);
@@ -737,6 +782,7 @@ int lbm_stats_from_raw(const double *raw, const double *centre, int ny, double c
 int lbm_set_graphs(lbm_t *h, int mode)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (mode < 0 || mode > 2) return fail(LBM_EINVAL, "mode must be 0 (off), 1 (on) or 2 (auto)");
     h->graph_mode = mode;
     if (mode == 0) graph_drop(h);
@@ -754,6 +800,7 @@ static KParams read_params(lbm_s *h)
 int lbm_get_macros(lbm_t *h, float *rho_dev, float *u_dev)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->inited) return fail(LBM_ESTATE, "lbm_get_macros before lbm_init / lbm_set_macros");
     KParams p = read_params(h);
     p.rho_out = rho_dev; p.u_out = u_dev;
@@ -764,6 +811,7 @@ int lbm_get_macros(lbm_t *h, float *rho_dev, float *u_dev)
 int lbm_get_macros_host(lbm_t *h, float *rho_host, float *u_host)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->inited) return fail(LBM_ESTATE, "lbm_get_macros_host before lbm_init / lbm_set_macros");
     const size_t plane = (size_t)h->nx * h->ny;
     float *stg = reinterpret_cast<float *>(h->ws + h->L.staging);
@@ -782,13 +830,30 @@ int lbm_get_macros_host(lbm_t *h, float *rho_host, float *u_host)
                 CU_TRY(cudaMemcpyAsync(u_host + (size_t)h->N * a + plane * z0, stg + cnt * (1 + a), cnt * 4,
                                        cudaMemcpyDeviceToHost, h->stream));
     }
+    int flag = 0;
+    CU_TRY(cudaMemcpyAsync(&flag, h->ws + h->L.flag, 4, cudaMemcpyDeviceToHost, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream));
+    if (flag) return fail(LBM_EDIVERGED, "non-finite density in the sampled field");
+    return LBM_OK;
+}
+
+int lbm_diverged(lbm_t *h, int *flag_out)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_diverged before lbm_bind");
+    int flag = 0;
+    CU_TRY(cudaMemcpyAsync(&flag, h->ws + h->L.flag, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    if (flag_out) *flag_out = flag;
+    if (flag) return fail(LBM_EDIVERGED, "a non-finite density was seen by lbm_get_macros* or the statistics reduction");
     return LBM_OK;
 }
 
 int lbm_get_state(lbm_t *h, float *out_dev)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->inited) return fail(LBM_ESTATE, "lbm_get_state before lbm_init / lbm_set_macros");
     if (!out_dev) return fail(LBM_EINVAL, "output is NULL");
     KParams p = read_params(h);
@@ -798,6 +863,44 @@ int lbm_get_state(lbm_t *h, float *out_dev)
     else state_kernel<2><<<blocks, 256, 0, h->stream>>>(p, out_dev);
     h->launches++;
     CU_TRY(cudaGetLastError());
+    return LBM_OK;
+}
+
+template <int V>
+static cudaError_t launch_setstate_v(lbm_s *h, const KParams &p, const float *in, bool odd)
+{
+    dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY * h->nchunk));
+    if (h->mask) {
+        if (!h->aa) setstate_kernel<V, WR_LOCAL, true><<<grid, block, 0, h->stream>>>(p, in);
+        else if (odd) setstate_kernel<V, WR_LOCAL_OPP, true><<<grid, block, 0, h->stream>>>(p, in);
+        else setstate_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p, in);
+    } else if (!h->aa) setstate_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p, in);
+    else if (odd) setstate_kernel<V, WR_LOCAL_OPP><<<grid, block, 0, h->stream>>>(p, in);
+    else setstate_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p, in);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+int lbm_set_state(lbm_t *h, const float *in_dev, long long t)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_state before lbm_bind");
+    if (!in_dev) return fail(LBM_EINVAL, "input is NULL");
+    if (t < 0) return fail(LBM_EINVAL, "t must be >= 0");
+    fill_params(h);
+    KParams p = h->kp;
+    const bool odd = (t & 1) != 0;
+    if (!h->aa && odd) p.dst = reinterpret_cast<float *>(h->ws + h->L.pops2);   // the lattice holding state t
+    else p.dst = p.src;
+    cudaError_t e;
+    switch (h->V) {
+    case 4: e = launch_setstate_v<4>(h, p, in_dev, odd); break;
+    case 2: e = launch_setstate_v<2>(h, p, in_dev, odd); break;
+    default: e = launch_setstate_v<1>(h, p, in_dev, odd); break;
+    }
+    CU_TRY(e);
+    h->t = t; h->inited = true;
     return LBM_OK;
 }
 
@@ -812,6 +915,7 @@ int lbm_stats_accumulate(lbm_t *h, int every)
 int lbm_stats_reset(lbm_t *h)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_reset before lbm_bind");
     return stats_reset_impl(h);
 }
@@ -819,6 +923,7 @@ int lbm_stats_reset(lbm_t *h)
 int lbm_stats_read(lbm_t *h, double *out, long long *nsamples)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_stats_read before lbm_bind");
     if (!out) return fail(LBM_EINVAL, "out is NULL");
     std::vector<double> acc((size_t)h->ny * NSTAT);
@@ -860,6 +965,7 @@ int lbm_set_kernel_timing(lbm_t *h, int on)
 int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
     if (!h->bound) return fail(LBM_ESTATE, "lbm_kernel_timing_read before lbm_bind");
     CU_TRY(cudaStreamSynchronize(h->stream));
     double tot = 0.0;
@@ -877,8 +983,12 @@ int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches)
 void lbm_destroy(lbm_t *h)
 {
     if (!h) return;
-    graph_drop(h);
-    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+    {
+        DevGuard dg(h);
+        graph_drop(h);
+        for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+        h->ev.clear();
+    }
     delete h;
 }
 

@@ -64,7 +64,6 @@ struct KParams {
     // physics (fp32 copies)
     float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
     float Fbx, Fby, Fbz;        // body force density F_b
-    double Fb64[3];             // the same in fp64 (momentum channel)
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
@@ -76,6 +75,7 @@ struct KParams {
     const float *shift;         // [ny][4] accumulation centre (u0, v0, w0, -), may be NULL
     // macros / init
     float *rho_out, *u_out;
+    int *diverged;              // set to 1 by macros_kernel when it sees a non-finite density
     const float *rho_in, *u_in; // init from fields (NULL -> synthetic)
     const float *uprof;         // [ny] synthetic profile U(y_j)
     double noise_amp;           // noise_frac * U_ref
@@ -779,6 +779,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
         if (!solid) stats_add(s, m);
         r[k] = solid ? 1.0f : m.rho;             // solid cells report the rest state
         ux[k] = solid ? 0.f : m.ux; uy[k] = solid ? 0.f : m.uy; uz[k] = solid ? 0.f : m.uz;
+        if (!isfinite(r[k]) && p.diverged) *p.diverged = 1;   // LBM_EDIVERGED sentinel
     }
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
     if (p.rho_out) stv<V>(p.rho_out + off, r);
@@ -850,6 +851,24 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) init_kernel(const K
             g[i][k] = wgt * (e0 + rho * cu * (3.0f + 4.5f * cu));
         });
     }
+    store_all<V, WM, MASK>(p, c, g, S);
+}
+
+// Plain "state k" populations [19][N] (the layout lbm_get_state writes) into whatever
+// representation the storage scheme / time parity wants: WR_LOCAL (two-lattice), WR_LOCAL_OPP
+// (AA, t odd), WR_PUSH (AA, t even).  Solid cells are written as the rest state.
+template <int V, int WM, bool MASK = false>
+__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) setstate_kernel(const KParams p, const float *in)
+{
+    const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
+    unsigned long long S = 0ull;
+    if constexpr (MASK) S = solid_gather<V>(p, c, solid_nb_word(p, c));
+    float g[Q][V];
+    const long long cell0 = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        ldv<V>(in + (long long)i * p.N + cell0, g[i]);
+    });
     store_all<V, WM, MASK>(p, c, g, S);
 }
 

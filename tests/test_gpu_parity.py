@@ -227,16 +227,75 @@ def test_cfg1_200_steps(orc, gpu, aa):
     assert abs(sg[:, 9].mean() - 1.0) < 1e-6
 
 
+_ORACLE_CACHE = {}
+
+
+def _oracle_macros_at(orc, cfg, seed, steps):
+    """(rho, u) of the oracle's sample S_steps for (config, seed); computed once per session and
+    shared by the storage variants (the oracle run is the expensive side)."""
+    key = (cfg["name"], seed, steps)
+    if key not in _ORACLE_CACHE:
+        c = dict(cfg)
+        c["seed"] = seed
+        o = orc.Oracle.from_config(c)
+        o.init_from_config(c)
+        o.step(steps)
+        _ORACLE_CACHE[key] = o.get_macros()
+        del o
+    return _ORACLE_CACHE[key]
+
+
+def _gpu_err_vs(orc, gpu, cfg, seed, steps, aa):
+    import torch
+    ro, uo = _oracle_macros_at(orc, cfg, seed, steps)
+    c = dict(cfg)
+    c["seed"] = seed
+    g = gpu.Lbm.from_config(c, aa=aa)
+    g.init(seed)
+    g.step(steps)
+    rg, ug = g.get_macros()
+    torch.cuda.synchronize()
+    er = float((rg.double().cpu() - torch.from_numpy(ro)).abs().max())
+    eu = float((ug.double().cpu() - torch.from_numpy(uo)).abs().max())
+    variant = g.variant
+    g.close()
+    return er, eu, variant
+
+
+# north_star: "Over 100 steps, the macroscopic rho and u must satisfy max|delta| <= 1e-5 relative
+# to the bulk velocity".  Several seeds per config: the flow amplifies rounding differences, so
+# the margin is a property of the realisation, not only of the arithmetic.
 @pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
-def test_cfg2_100_steps(orc, gpu, aa):
-    cfg = wl.get("cfg2")
-    o, g = _pair(orc, gpu, cfg, aa, 0)
+@pytest.mark.parametrize("seed", [12345, 1, 20220630, 987654321])
+def test_cfg1_100_steps_seeds(orc, gpu, aa, seed):
+    cfg = wl.get("cfg1")
     tol = TOL_REL * cfg["u_bulk"]
-    o.step(100)
-    g.step(100)
-    er, eu = _macro_err(o, g)
-    print(f"cfg2 {g.variant} step 100: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
+    er, eu, variant = _gpu_err_vs(orc, gpu, cfg, seed, 100, aa)
+    print(f"cfg1 {variant} seed {seed} step 100: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
     assert er <= tol and eu <= tol
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("seed", [12345, 1, 20220630])
+def test_cfg2_100_steps(orc, gpu, aa, seed):
+    cfg = wl.get("cfg2")
+    tol = TOL_REL * cfg["u_bulk"]
+    er, eu, variant = _gpu_err_vs(orc, gpu, cfg, seed, 100, aa)
+    print(f"cfg2 {variant} seed {seed} step 100: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
+    assert er <= tol and eu <= tol
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+def test_cfg3_100_steps(orc, gpu, aa):
+    """BASELINE.json:configs[2]: the first config with the Lalic-Mihailovic canopy (PAPER.md:L105-115,
+    Eqs. 14-15) at full width, 512x128x256.  The oracle side is ~5 GB and runs once."""
+    cfg = wl.get("cfg3")
+    tol = TOL_REL * cfg["u_bulk"]
+    er, eu, variant = _gpu_err_vs(orc, gpu, cfg, cfg["seed"], 100, aa)
+    print(f"cfg3 {variant} step 100: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol:.1e})")
+    assert er <= tol and eu <= tol
+    if aa:
+        _ORACLE_CACHE.pop((cfg["name"], cfg["seed"], 100), None)   # 0.5 GB of fp64 fields
 
 
 # ---------------------------------------------------------------------------------------------
@@ -449,3 +508,121 @@ def test_step_before_init_is_an_error(gpu):
     with pytest.raises(gpu.LbmError) as e:
         g.step(1)
     assert e.value.code == gpu.LBM_ESTATE
+
+
+# ---------------------------------------------------------------------------------------------
+# lbm_set_state: checkpoint / restart, and pin P16 through the C ABI
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("t0", [4, 7])
+@pytest.mark.parametrize("solid", [False, True])
+def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
+    """get_state -> set_state(t) into a fresh handle -> step continues the run bit for bit."""
+    import torch
+    cfg = wl.small(nx=64, ny=10, nz=6)
+    if solid:
+        cfg["solid"] = _solid_mask("boxes", 64, 10, 6)
+    a = gpu.Lbm.from_config(cfg, aa=aa)
+    a.init(cfg["seed"])
+    a.step(t0)
+    ck = a.get_state().clone()
+    a.step(5)
+    want = a.get_state().cpu().numpy()
+    b = gpu.Lbm.from_config(cfg, aa=aa)
+    b.set_state(ck, t0)
+    assert b.time == t0
+    assert np.array_equal(b.get_state().cpu().numpy(), ck.cpu().numpy())
+    b.step(5)
+    torch.cuda.synchronize()
+    assert b.time == a.time and np.array_equal(b.get_state().cpu().numpy(), want)
+    ra, ua = a.get_macros()
+    rb, ub = b.get_macros()
+    assert torch.equal(ra, rb) and torch.equal(ua, ub)
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("t0", [0, 1])
+def test_p16_known_pi_neq_through_the_c_abi(orc, gpu, aa, t0):
+    """Pin P16 (tests/test_oracle_pins.py) on the CUDA path: a periodic uniform state with a known
+    Pi_neq = A relaxes by (1 - 1/tau_t) in one step (Eq. 11).  t0 selects
+    the AA parity (even step / odd step kernel)."""
+    import torch
+    c, w, _, _ = orc.tables()
+    c = c.astype(float)
+    rng = np.random.default_rng(61)
+    nx, ny, nz = 32, 4, 3
+    flags = gpu.bc_flags("periodic", "periodic", aa=aa)
+    for trial in range(6):
+        B = rng.normal(size=(3, 3))
+        A = 0.5 * (B + B.T)
+        A -= np.trace(A) / 3 * np.eye(3)
+        A *= 3e-3 / np.sqrt(np.sum(A * A))
+        rho = rng.uniform(0.93, 1.07)
+        u = rng.uniform(-0.1, 0.1, 3) + np.array([0.05, 0.0, 0.0])
+        nu, Cs = 10 ** rng.uniform(-4, -2.5), 0.17
+        tau0 = 3 * nu + 0.5
+        cu = c @ u
+        feq = w * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u @ u))
+        fneq = w * 4.5 * np.einsum("iab,ab->i", np.einsum("ia,ib->iab", c, c) - np.eye(3) / 3, A)
+        tau_t = 0.5 * (tau0 + np.sqrt(tau0 ** 2 + 18 * np.sqrt(2) * Cs ** 2 * np.sqrt(np.sum(A * A)) / rho))
+        want = feq + (1 - 1 / tau_t) * fneq - w
+        g = gpu.Lbm(nx, ny, nz, nu, Cs, flags=flags)
+        st = torch.from_numpy(np.broadcast_to((feq + fneq - w)[:, None, None, None], (19, nz, ny, nx))
+                              .astype(np.float32).copy()).cuda()
+        g.set_state(st, t0)
+        g.step(1)
+        got = g.get_state().double().cpu().numpy()
+        err = np.abs(got - want[:, None, None, None]).max()
+        teeth = np.abs((1 / tau0 - 1 / tau_t) * fneq).max()
+        assert err <= 3e-8 and teeth > 30 * 3e-8, (err, teeth)
+        g.close()
+
+
+def test_divergence_is_reported(gpu):
+    """A deliberately unstable run (nu = 1e-6, Cs = 0, large noise at Ma ~ 0.5) blows up; the
+    library must say so: LBM_EDIVERGED from get_macros_host / stats_read, lbm_diverged() true."""
+    for aa in (False, True):
+        g = gpu.Lbm(32, 16, 16, 1e-6, 0.0, body_force=(1e-3, 0, 0),
+                    flags=gpu.bc_flags("bounce_back", "free_slip", aa=aa))
+        g.set_init(gpu.INIT_POWER_LAW, 0.3, 1.5)
+        g.init(3)
+        assert not g.diverged()
+        g.stats_accumulate(1)
+        for _ in range(40):
+            g.step(50)
+            g.get_macros()
+            if g.diverged():
+                break
+        assert g.diverged()
+        with pytest.raises(gpu.LbmError) as e:
+            g.get_macros_host()
+        assert e.value.code == gpu.LBM_EDIVERGED
+        with pytest.raises(gpu.LbmError) as e:
+            g.stats_read()
+        assert e.value.code == gpu.LBM_EDIVERGED
+        g.init(3)                                  # re-initialising clears the flag
+        assert not g.diverged()
+        g.close()
+
+
+def test_chunked_host_transfers(orc, gpu, monkeypatch):
+    """Host transfers through a staging area smaller than the lattice (forced with
+    LBM_STAGING_BYTES): every row of every chunk is initialised and read back, also when the
+    block covers several rows (TY > 1)."""
+    monkeypatch.setenv("LBM_STAGING_BYTES", str(16 * 16 * 12 * 3))       # 3 planes of 16 x 12
+    cfg = wl.small(nx=16, ny=12, nz=10)
+    o = orc.Oracle.from_config(cfg)
+    rho, u = o.init_field(cfg["init"]["kind"], cfg["init"]["U_ref"], cfg["init"]["noise_frac"], 5)
+    o.set_macros(rho, u)
+    w = _weights(orc)
+    for aa in (False, True):
+        g = gpu.Lbm.from_config(cfg, aa=aa)
+        assert "x" in g.variant and int(g.variant.split("x")[-1]) > 1    # several rows per block
+        with pytest.raises(gpu.LbmError):
+            g.set_launch_shape(4, 8)                                      # 8 does not divide ny = 12
+        g.set_macros_host(rho.astype(np.float32), u.astype(np.float32))
+        assert _state_err(o, g, w) <= 5e-8
+        rh, uh = g.get_macros_host()
+        rd, ud = g.get_macros()
+        assert np.array_equal(rh, rd.cpu().numpy()) and np.array_equal(uh, ud.cpu().numpy())
+        g.close()
