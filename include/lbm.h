@@ -111,6 +111,18 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host);
  * Errors: LBM_ENOMEM (bytes < lbm_workspace_bytes or pointer not 256-B aligned), LBM_ECUDA. */
 int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream);
 
+/* Momentum reference of the collision arithmetic: jx_ref_host, host,
+ * ny doubles, an estimate of the mean streamwise momentum rho*u_x of each row (NULL = 0).  The
+ * kernels evaluate the momentum channel of the collision about it, which removes the rounding of
+ * the mean flow from the fp32 result; it never changes what is computed in exact arithmetic, any
+ * finite profile is valid, and the closer it is to the flow the smaller the rounding error.
+ * lbm_init installs the synthetic initial profile; lbm_set_macros* and lbm_set_state leave the
+ * reference as it is.  lbm_get_reference_profile returns the profile in use (as rounded by the
+ * library; setting it again reproduces it exactly), so that a checkpoint of lbm_get_state + lbm_time
+ * + this profile restarts a run bit for bit.  Call after lbm_bind; both synchronise the stream. */
+int lbm_set_reference_profile(lbm_t *h, const double *jx_ref_host);
+int lbm_get_reference_profile(lbm_t *h, double *jx_ref_host);
+
 /* Choose the synthetic initial field used by lbm_init (R16): rho = 1,
  * u = U(y_j) e_x + noise_frac*U_ref*(2r-1) per component, r = rand01(seed, 3*cell+comp). */
 int lbm_set_init(lbm_t *h, int kind, double U_ref, double noise_frac);
@@ -213,6 +225,16 @@ long long lbm_launch_count(const lbm_t *h);
  * staging area, 256 MB unless the environment variable LBM_STAGING_BYTES says otherwise).  Call
  * before the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
+
+/* Data-movement path of the step kernel.  mode is a bit mask of the step kinds that stream through
+ * the Tensor Memory Accelerator (lbm_tma.cuh: cp.async.bulk.tensor tile loads/stores whose box
+ * coordinates carry the streaming shift) instead of per-thread 128-bit accesses: bit 0 the AA even
+ * step, bit 1 the AA odd step, bit 2 the two-lattice pull step; 0 = none.  rows = y rows per
+ * 256-cell tile (1, 2 or 4, must divide ny; 0 = keep).  Both paths compute the same thing with the
+ * same per-cell arithmetic.  Available with 4 cells per thread, nx % 256 == 0 and no solid mask
+ * (LBM_EINVAL otherwise); the environment variable LBM_TMA="mode[,rows]" sets the default of new
+ * handles.  Call before or between lbm_step calls. */
+int lbm_set_tma(lbm_t *h, int mode, int rows);
 
 /* Measurement hook (bench.py "roofline"): with on != 0, lbm_step brackets every step-kernel
  * launch (the fused S1-S8 kernel only, not the stage-2 reduction) with a pair of CUDA events on

@@ -41,7 +41,7 @@ SYMBOLS = [
     "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
-    "lbm_set_state", "lbm_diverged",
+    "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma",
 ]
 
 
@@ -91,6 +91,9 @@ def lib():
         L.lbm_get_state.argtypes = [vp, fp]
         L.lbm_set_state.argtypes = [vp, fp, C.c_longlong]
         L.lbm_diverged.argtypes = [vp, C.POINTER(C.c_int)]
+        L.lbm_set_reference_profile.argtypes = [vp, dp]
+        L.lbm_get_reference_profile.argtypes = [vp, dp]
+        L.lbm_set_tma.argtypes = [vp, C.c_int, C.c_int]
         L.lbm_time.argtypes = [vp]
         L.lbm_time.restype = C.c_longlong
         L.lbm_launch_count.argtypes = [vp]
@@ -351,6 +354,25 @@ class Lbm:
 
         out = torch.empty((19,) + self.shape, dtype=torch.float32, device=self.device)
         _check(lib().lbm_get_state(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def set_tma(self, mode: int, rows: int = 0):
+        """Which step kinds stream through the TMA unit (bit 0 AA even, 1 AA odd, 2 pull); rows per tile."""
+        _check(lib().lbm_set_tma(self._h, int(mode), int(rows)))
+
+    def set_reference_profile(self, jx_ref=None):
+        """Per-row momentum reference of the collision arithmetic (rounding only); None = 0."""
+        if jx_ref is None:
+            _check(lib().lbm_set_reference_profile(self._h, None))
+            return
+        r = np.ascontiguousarray(jx_ref, dtype=np.float64)
+        if r.shape != (self.ny,):
+            raise ValueError("jx_ref must have ny entries")
+        _check(lib().lbm_set_reference_profile(self._h, _dp(r)))
+
+    def get_reference_profile(self) -> np.ndarray:
+        out = np.zeros(self.ny)
+        _check(lib().lbm_get_reference_profile(self._h, _dp(out)))
         return out
 
     def set_state(self, f_minus_w, t: int = 0):

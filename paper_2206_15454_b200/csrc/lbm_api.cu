@@ -2,6 +2,7 @@
 // layout, kernel dispatch.  No torch types; the caller owns the device workspace and the stream.
 #include "../../include/lbm.h"
 #include "lbm_kernels.cuh"
+#include "lbm_tma.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -49,7 +50,7 @@ static size_t staging_budget()
 }
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, flag, solid, solid_nb, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, staging, total;
     int stage_planes;
 };
 
@@ -60,11 +61,13 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     size_t off = 0;
     L.pops = off; off = align_up(off + (size_t)Q * N * 4, 256);
     L.pops2 = off; if (!aa) off = align_up(off + (size_t)Q * N * 4, 256);
-    L.partial = off; off = align_up(off + (size_t)ny * NSTAT * nz * MAX_NCHUNK * 4, 256);
+    const int pmax = (nx / TMA_BOX > MAX_NCHUNK) ? nx / TMA_BOX : MAX_NCHUNK;
+    L.partial = off; off = align_up(off + (size_t)ny * NSTAT * nz * pmax * 4, 256);
     L.acc = off; off = align_up(off + (size_t)ny * NSTAT * 8, 256);
     L.shift = off; off = align_up(off + (size_t)ny * 4 * 4, 256);
     L.cda = off; off = align_up(off + (size_t)ny * 4, 256);
     L.uprof = off; off = align_up(off + (size_t)ny * 4, 256);
+    L.jref = off; off = align_up(off + (size_t)ny * 4, 256);
     L.flag = off; off += 256;
     L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     L.solid_nb = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
@@ -91,6 +94,12 @@ struct lbm_s {
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
     std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
     int V, TX, TY, nchunk;
+    int pchunks;                // x chunks per row in the layout of the statistics partials
+    // TMA data path (lbm_tma.cuh): which step kinds use it (bit 0 AA even, 1 AA odd, 2 two-lattice
+    // pull) and rows per tile; maps of the two population arrays (box 256 x 1 x 1 x 1)
+    bool tma_ok;
+    int tma_mode, tma_rows;
+    CUtensorMap map_a, map_b;
     Layout L;
     char *ws;
     cudaStream_t stream;
@@ -132,6 +141,33 @@ static void graph_drop(lbm_s *h)
 {
     if (h->gexec) cudaGraphExecDestroy(h->gexec);
     h->gexec = nullptr;
+}
+
+constexpr int TMA_DEFAULT_MODE = 7;
+
+static void set_variant(lbm_s *h)
+{
+    char tma[32] = "";
+    if (h->tma_mode) snprintf(tma, sizeof(tma), "/tma%dx%d", h->tma_mode, h->tma_rows);
+    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d%s", h->aa ? "aa" : "pull2", h->V, h->TX, h->TY, tma);
+}
+
+// The statistics partials are laid out with `pchunks` x chunks per row: the larger of the
+// chunkings of the kernels in use.  When it changes the buffer is cleared (entries no kernel
+// writes must read as zero in the stage-2 sum).
+static int set_pchunks(lbm_s *h)
+{
+    int pc = h->nchunk;
+    if (h->tma_mode && h->nx / TMA_BOX > pc) pc = h->nx / TMA_BOX;
+    if (pc != h->pchunks) {
+        h->pchunks = pc;
+        graph_drop(h);
+        if (h->bound) {
+            h->kp.pchunks = pc;
+            CU_TRY(cudaMemsetAsync(h->ws + h->L.partial, 0, h->L.acc - h->L.partial, h->stream));
+        }
+    }
+    return LBM_OK;
 }
 
 static bool valid_top_bottom(uint32_t bc, int *bot, int *top)
@@ -237,6 +273,21 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
         return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
     }
     h->nchunk = (nx / V) / h->TX;
+    h->tma_ok = (V == 4) && (nx % TMA_BOX == 0) && !h->mask;
+    h->tma_rows = (ny % 2 == 0) ? 2 : 1;
+    h->tma_mode = 0;
+    if (h->tma_ok) {
+        h->tma_mode = TMA_DEFAULT_MODE;
+        const char *e = getenv("LBM_TMA");          // tuning / A-B override: "mode[,rows]"
+        if (e && *e) {
+            int m = 0, r = 0;
+            const int got = sscanf(e, "%d,%d", &m, &r);
+            if (got >= 1 && m >= 0 && m <= 7) h->tma_mode = m;
+            if (got >= 2 && (r == 1 || r == 2 || r == 4) && ny % r == 0) h->tma_rows = r;
+        }
+    }
+    h->pchunks = h->nchunk;
+    if (h->tma_mode && nx / TMA_BOX > h->pchunks) h->pchunks = nx / TMA_BOX;
     h->zlo = h->halo ? 1 : 0; h->zhi = h->halo ? nz - 1 : nz;
     h->zg0 = h->halo ? -1 : 0; h->nzg = h->halo ? nz - 2 : nz;
     h->nfluid.assign(ny, (double)nx * (h->zhi - h->zlo));
@@ -247,7 +298,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->graph_mode = 2; h->gexec = nullptr; h->g_steps = 0; h->g_parity = 0; h->g_every = 0;
     h->g_launches = 0; h->g_samples = 0;
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
-    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", V, h->TX, h->TY);
+    set_variant(h);
     *out = h;
     return LBM_OK;
 }
@@ -264,8 +315,8 @@ int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
     graph_drop(h);
     h->TX = tx; h->TY = ty; h->nchunk = W / tx;
     h->kp.nchunk = h->nchunk;
-    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d", h->aa ? "aa" : "pull2", h->V, h->TX, h->TY);
-    return LBM_OK;
+    set_variant(h);
+    return set_pchunks(h);
 }
 
 static void fill_params(lbm_s *h)
@@ -274,12 +325,13 @@ static void fill_params(lbm_s *h)
     memset(&p, 0, sizeof(p));
     p.src = reinterpret_cast<float *>(h->ws + h->L.pops);
     p.dst = h->aa ? p.src : reinterpret_cast<float *>(h->ws + h->L.pops2);
-    p.nx = h->nx; p.ny = h->ny; p.nz = h->nz; p.nchunk = h->nchunk; p.N = h->N;
+    p.nx = h->nx; p.ny = h->ny; p.nz = h->nz; p.nchunk = h->nchunk; p.pchunks = h->pchunks; p.N = h->N;
     const double tau0 = 3.0 * h->nu + 0.5;              // R3
     p.tau0 = (float)tau0; p.tau0sq = (float)(tau0 * tau0);
     p.ksmag = (float)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs); // R9: C_smag = Cs^2
     p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
     p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
+    p.jref = reinterpret_cast<const float *>(h->ws + h->L.jref);
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
     {
         // lid populations f_eq,i(1, U_top) - w_i (Eq. 3) of the five directions with c_y = -1
@@ -300,6 +352,34 @@ static void fill_params(lbm_s *h)
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
     p.z0 = 0; p.z1 = h->nz; p.zoff = 0; p.Nio = h->N;
     p.zg0 = h->zg0; p.nzg = h->nzg;
+    p.zv0 = h->zlo; p.zv1 = h->zhi;
+}
+
+// Tensor map of one population array viewed as a rank-4 fp32 tensor {x, y, z, slot} with a box of
+// one 256-cell row segment.  cuTensorMapEncodeTiled is a driver entry point; it is looked up
+// through the runtime so that the library does not link against libcuda.
+static int make_tensor_map(lbm_s *h, void *base, CUtensorMap *out)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        CU_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (q != cudaDriverEntryPointSuccess || !fn) return fail(LBM_ECUDA, "cuTensorMapEncodeTiled is not available");
+        encode = reinterpret_cast<encode_fn>(fn);
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)Q};
+    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * 4, (cuuint64_t)h->nx * h->ny * 4, (cuuint64_t)h->N * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)TMA_BOX, 1, 1, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(LBM_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return LBM_OK;
 }
 
 int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
@@ -320,12 +400,18 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     h->ws = static_cast<char *>(dev_workspace);
     h->stream = static_cast<cudaStream_t>(cuda_stream);
     fill_params(h);
+    if (h->tma_ok) {
+        int rc = make_tensor_map(h, h->ws + h->L.pops, &h->map_a);
+        if (rc == LBM_OK && !h->aa) rc = make_tensor_map(h, h->ws + h->L.pops2, &h->map_b);
+        if (rc != LBM_OK) return rc;
+    }
     std::vector<float> cda(h->ny);
     for (int j = 0; j < h->ny; ++j) cda[j] = (float)(h->Cd * h->lad[j]);
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.cda, cda.data(), h->ny * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.acc, 0, (size_t)h->ny * NSTAT * 8, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
+    CU_TRY(cudaMemsetAsync(h->ws + h->L.jref, 0, (size_t)h->ny * 4, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.partial, 0, h->L.acc - h->L.partial, h->stream));
     if (h->mask) {
         const size_t mbytes = (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4;
@@ -455,9 +541,43 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
     }
 }
 
+template <int RM, int WM, bool S, int R>
+static cudaError_t launch_tma_r(lbm_s *h, const KParams &p, const CUtensorMap &ms, const CUtensorMap &md)
+{
+    static bool attr_set = false;
+    const int smem = Q * R * TMA_BOX * 4;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(step_tma_kernel<RM, WM, S, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    dim3 block(TMA_TX, R), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / R * (h->nx / TMA_BOX)));
+    step_tma_kernel<RM, WM, S, R><<<grid, block, smem, h->stream>>>(p, ms, md);
+    h->launches++;
+    return cudaGetLastError();
+}
+template <int RM, int WM, bool S>
+static cudaError_t launch_tma(lbm_s *h, const KParams &p)
+{
+    // the maps follow the src/dst roles of this step (two-lattice: they swap every step)
+    const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
+    const CUtensorMap &ms = swapped ? h->map_b : h->map_a;
+    const CUtensorMap &md = h->aa ? h->map_a : (swapped ? h->map_a : h->map_b);
+    switch (h->tma_rows) {
+    case 4: return launch_tma_r<RM, WM, S, 4>(h, p, ms, md);
+    case 2: return launch_tma_r<RM, WM, S, 2>(h, p, ms, md);
+    default: return launch_tma_r<RM, WM, S, 1>(h, p, ms, md);
+    }
+}
+
 template <int V, bool S>
 static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
 {
+    if (V == 4 && h->tma_mode) {
+        if (!h->aa) { if (h->tma_mode & 4) return launch_tma<RD_PULL, WR_LOCAL, S>(h, p); }
+        else if ((h->t & 1) == 0) { if (h->tma_mode & 1) return launch_tma<RD_LOCAL, WR_LOCAL_OPP, S>(h, p); }
+        else if (h->tma_mode & 2) return launch_tma<RD_PULL_OPP, WR_PUSH, S>(h, p);
+    }
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / h->TY * h->nchunk));
     if (h->mask) {
         if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S, true><<<grid, block, 0, h->stream>>>(p);
@@ -482,7 +602,7 @@ static cudaError_t launch_stage2(lbm_s *h, int mode)
 {
     dim3 grid(h->ny, NSTAT);
     stats_stage2_kernel<<<grid, 256, 0, h->stream>>>(
-        reinterpret_cast<const float *>(h->ws + h->L.partial), (long long)h->nz * h->nchunk,
+        reinterpret_cast<const float *>(h->ws + h->L.partial), (long long)h->nz * h->pchunks,
         reinterpret_cast<double *>(h->ws + h->L.acc), reinterpret_cast<float *>(h->ws + h->L.shift), mode,
         1.0 / ((double)h->nx * h->nz), reinterpret_cast<int *>(h->ws + h->L.flag));
     h->launches++;
@@ -507,6 +627,50 @@ static int stats_reset_impl(lbm_s *h)
     return LBM_OK;
 }
 
+// r_j = J0_j / 12 with 16 significant bits, so that 2 r (axis populations) and 12 r (= J0) are
+// exact in fp32 (kernels: mom_ref_shift).
+static int upload_reference(lbm_s *h, const double *jx_ref)
+{
+    std::vector<float> r(h->ny, 0.f);
+    if (jx_ref)
+        for (int j = 0; j < h->ny; ++j) {
+            float v = (float)(jx_ref[j] / 12.0);
+            uint32_t b;
+            memcpy(&b, &v, 4);
+            b &= 0xFFFFFF00u;
+            memcpy(&v, &b, 4);
+            r[j] = std::isfinite(v) ? v : 0.f;
+        }
+    graph_drop(h);
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.jref, r.data(), h->ny * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_set_reference_profile(lbm_t *h, const double *jx_ref_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_reference_profile before lbm_bind");
+    if (jx_ref_host)
+        for (int j = 0; j < h->ny; ++j)
+            if (!std::isfinite(jx_ref_host[j])) return fail(LBM_EINVAL, "jx_ref[%d] is not finite", j);
+    return upload_reference(h, jx_ref_host);
+}
+
+int lbm_get_reference_profile(lbm_t *h, double *jx_ref_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_get_reference_profile before lbm_bind");
+    if (!jx_ref_host) return fail(LBM_EINVAL, "output is NULL");
+    std::vector<float> r(h->ny);
+    CU_TRY(cudaMemcpyAsync(r.data(), h->ws + h->L.jref, h->ny * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    for (int j = 0; j < h->ny; ++j) jx_ref_host[j] = 12.0 * (double)r[j];
+    return LBM_OK;
+}
+
 static int upload_profile(lbm_s *h)
 {
     std::vector<float> up(h->ny);
@@ -519,7 +683,9 @@ static int upload_profile(lbm_s *h)
     }
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.uprof, up.data(), h->ny * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream));
-    return LBM_OK;
+    // the synthetic profile (rho = 1) is also the momentum reference of the run it starts
+    std::vector<double> ref(up.begin(), up.end());
+    return upload_reference(h, ref.data());
 }
 
 int lbm_init(lbm_t *h, uint64_t seed)
@@ -777,6 +943,22 @@ int lbm_stats_from_raw(const double *raw, const double *centre, int ny, double c
         r[9] = a[9] / count;
     }
     return LBM_OK;
+}
+
+int lbm_set_tma(lbm_t *h, int mode, int rows)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (mode < 0 || mode > 7) return fail(LBM_EINVAL, "mode is a bit mask 0..7");
+    if (mode && !h->tma_ok)
+        return fail(LBM_EINVAL, "the TMA path needs 4 cells per thread, nx %% 256 == 0 and no solid mask");
+    if (rows != 0 && !((rows == 1 || rows == 2 || rows == 4) && h->ny % rows == 0))
+        return fail(LBM_EINVAL, "rows per tile must be 1, 2 or 4 and divide ny");
+    graph_drop(h);
+    h->tma_mode = mode;
+    if (rows) h->tma_rows = rows;
+    set_variant(h);
+    return set_pchunks(h);
 }
 
 int lbm_set_graphs(lbm_t *h, int mode)

@@ -60,11 +60,13 @@ struct KParams {
     float *dst;          // population array written (== src for AA)
     int nx, ny, nz;
     int nchunk;          // blocks per x row
+    int pchunks;         // x chunks per row in the layout of `partial` (>= nchunk of any kernel in use)
     long long N;
     // physics (fp32 copies)
     float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
     float Fbx, Fby, Fbz;        // body force density F_b
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
+    const float *jref;          // [ny] r_j = J0_j / 12: per-row momentum reference (see mom_ref_shift)
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
     const unsigned *solid_nb;   // the same mask dilated by one cell in x, y, z (host-built)
@@ -82,6 +84,7 @@ struct KParams {
     unsigned long long seed;
     int z0, z1;                 // z range of a launch (chunked host transfers; interior planes of a slab)
     int zg0, nzg;               // z slab: global z of local plane 0 and global nz (init recipe only)
+    int zv0, zv1;               // planes that hold the lattice proper ([1, nz-1) on a z slab: not the ghosts)
     long long zoff;             // element offset of plane z0 inside rho_in/u_in/rho_out/u_out
     long long Nio;              // component stride of u_in / u_out
 };
@@ -492,13 +495,37 @@ __device__ __forceinline__ float sqrt_approx(float x)
 struct Cell {
     float drho, rho, inv_rho;
     float jx, jy, jz;   // force-corrected momentum rho u = sum f c + F/2 (Eq. 6)
+    float jxr;          // jx - J0: the same about the row's momentum reference
     float ux, uy, uz;   // force-corrected velocity (the sample S)
     float Fx, Fy, Fz;   // total force density F_b + F_f
     float Pxx, Pyy, Pzz, Pxy, Pyz, Pxz; // sum g_i c c  (= Pi - I/3)
 };
 
+// Momentum reference (arithmetic form only).  With omega close to 2
+// the collision reflects the momentum channel, j* = (1 - w) m + w j, so a rounding error in the
+// computed j - the 10-term sum at the magnitude of the mean flow, the product 3 w j, the inexact
+// weights 1/18, 1/36 - returns doubled every step, and in a smooth flow with the same sign: a
+// drift proportional to |u| (measured 1e-5 |u| after 100 steps).  The linear odd part of any
+// reference equilibrium, ref_i = w_i 3 c_ix J0, passes through the collision unchanged
+// ((1 - w) ref + w ref = ref), so the x-moving populations are taken about it: g'_i = g_i - ref_i
+// before the moments, the collision acts on j' = j - J0 (small), and ref_i is added back in the
+// final sum.  J0 is a per-row constant with few mantissa bits (r = J0/12 = ref of a diagonal
+// population, 2r = ref of an axis population are exact); it changes rounding only, never the
+// exact-arithmetic result.
 template <int V>
-__device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V], int k, float cda)
+__device__ __forceinline__ void mom_ref_shift(float (&g)[Q][V], int k, float r)
+{
+    const float r1 = 2.0f * r;
+    g[1][k] -= r1; g[2][k] += r1;
+    g[7][k] -= r; g[8][k] += r;
+    g[9][k] -= r; g[10][k] += r;
+    g[11][k] -= r; g[12][k] += r;
+    g[13][k] -= r; g[14][k] += r;
+}
+
+// g: populations of the cell with mom_ref_shift(r) applied; r = J0 / 12 of the row.
+template <int V>
+__device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V], int k, float cda, float r)
 {
     Cell m;
     const float s1 = g[1][k] + g[2][k], d1 = g[1][k] - g[2][k];
@@ -524,7 +551,8 @@ __device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V]
     m.rho = 1.0f + m.drho;
     m.inv_rho = rcp_approx(m.rho);
     // Alg. 1: local momentum with the driving force (Eq. 6; R7)
-    m.jx = mx + 0.5f * p.Fbx;
+    m.jxr = mx + 0.5f * p.Fbx;
+    m.jx = m.jxr + 12.0f * r;
     m.jy = my + 0.5f * p.Fby;
     m.jz = mz + 0.5f * p.Fbz;
     m.Fx = p.Fbx; m.Fy = p.Fby; m.Fz = p.Fbz;
@@ -534,7 +562,7 @@ __device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V]
         const float coef = -cda * sqrt_approx(usx * usx + usy * usy + usz * usz);
         const float Ffx = coef * usx;
         // Alg. 1: correct the velocity with the forest force (explicit; R6)
-        m.jx += 0.5f * Ffx; m.Fx += Ffx;
+        m.jx += 0.5f * Ffx; m.jxr += 0.5f * Ffx; m.Fx += Ffx;
         if (p.drag_vector) {
             const float Ffy = coef * usy, Ffz = coef * usz;
             m.jy += 0.5f * Ffy; m.Fy += Ffy;
@@ -552,8 +580,10 @@ __device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V]
 //   F_i = (1 - w/2) w_i [ 3 c.F - 3 u.F + 9 (c.u)(c.F) ].
 // Per pair (i, opp i):  even part  w_i [ e0 + (c.u)(c.h) ],  h = 4.5 w j + 9 (1-w/2) F
 //                       odd part   w_i  c.k,                 k = 3 w j + 3 (1-w/2) F.
+// The x-moving populations come in about the momentum reference (mom_ref_shift) and go out
+// plain: their odd part is built from j' = jx - J0 and ref_i is added back in the same sum.
 template <int V>
-__device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m)
+__device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m, float r)
 {
     const float ux = m.ux, uy = m.uy, uz = m.uz;
     const float third_drho = m.drho * (1.0f / 3.0f);
@@ -574,7 +604,7 @@ __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int 
     const float e0 = w * (m.drho - 1.5f * uj) - 3.0f * gp * uF;
     const float a2 = 4.5f * w, b2 = 9.0f * gp, a1 = 3.0f * w, b1 = 3.0f * gp;
     const float hx = a2 * m.jx + b2 * m.Fx, hy = a2 * m.jy + b2 * m.Fy, hz = a2 * m.jz + b2 * m.Fz;
-    const float kx = a1 * m.jx + b1 * m.Fx, ky = a1 * m.jy + b1 * m.Fy, kz = a1 * m.jz + b1 * m.Fz;
+    const float kx = a1 * m.jxr + b1 * m.Fx, ky = a1 * m.jy + b1 * m.Fy, kz = a1 * m.jz + b1 * m.Fz;
     constexpr float W0 = 1.0f / 3.0f, W1 = 1.0f / 18.0f, W2 = 1.0f / 36.0f;
     g[0][k] = omw * g[0][k] + W0 * e0;
     // axis pairs: c.u = u_a, c.h = h_a, c.k = k_a
@@ -585,11 +615,11 @@ __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int 
         g[A][k] = omw * g[A][k] + (ev + od);        \
         g[B][k] = omw * g[B][k] + (ev - od);        \
     }
-    LBM_PAIR(1, 2, e1 + (W1 * ux) * hx, W1 * kx)
+    LBM_PAIR(1, 2, e1 + (W1 * ux) * hx, W1 * kx + 2.0f * r)
     LBM_PAIR(3, 4, e1 + (W1 * uy) * hy, W1 * ky)
     LBM_PAIR(5, 6, e1 + (W1 * uz) * hz, W1 * kz)
     const float vx = W2 * ux, vy = W2 * uy, vz = W2 * uz;   // weight folded into c.u
-    const float qx = W2 * kx, qy = W2 * ky, qz = W2 * kz;   // weight folded into c.k
+    const float qx = W2 * kx + r, qy = W2 * ky, qz = W2 * kz;   // weight folded into c.k (+ ref)
     LBM_PAIR(7, 8, e2 + (vx + vy) * (hx + hy), qx + qy)
     LBM_PAIR(9, 10, e2 + (vx - vy) * (hx - hy), qx - qy)
     LBM_PAIR(11, 12, e2 + (vx + vz) * (hx + hz), qx + qz)
@@ -604,7 +634,7 @@ __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int 
 // Columns: u, v, w, uu, vv, ww, uv, vw, uw, rho-1, all about the per-row centre `shift`.
 // The block owns blockDim.y row segments; each is reduced with warp shuffles (+ shared memory
 // across the warps of a segment) and stored, without atomics, to
-//   partial[(y*NSTAT + k) * (nz*nchunk) + z*nchunk + chunk].
+//   partial[(y*NSTAT + k) * (nz*pchunks) + z*pchunks + chunk].
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void stats_add(float (&s)[NSTAT], const Cell &m)
 {
@@ -629,42 +659,52 @@ __device__ __forceinline__ void stats_recentre(float (&s)[NSTAT], float n, float
     s[0] = a - n * u0; s[1] = b - n * v0; s[2] = c - n * w0;
 }
 
+// Sum each of the 10 columns over the 32 lanes of a warp: recursive-halving butterfly, 12
+// shuffles (split 5|5, 3|3, 2|2, 1|1, then a plain exchange).  Afterwards the lanes 0, 2, 4, 8,
+// 10 hold columns 0..4 and lanes 16, 18, 20, 24, 26 columns 5..9: `owner` lanes carry the total
+// of column `col` in `v4`.
+__device__ __forceinline__ void stats_warp_butterfly(const float (&s)[NSTAT], int lane, float &v4, bool &owner, int &col)
+{
+    const bool b16 = lane & 16, b8 = lane & 8, b4 = lane & 4, b2 = lane & 2;
+    float v1[6], v2[4], v3[2];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const float keep = b16 ? s[k + 5] : s[k], send = b16 ? s[k] : s[k + 5];
+        v1[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+    v1[5] = 0.f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const float keep = b8 ? v1[k + 3] : v1[k], send = b8 ? v1[k] : v1[k + 3];
+        v2[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    v2[3] = 0.f;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const float keep = b4 ? v2[k + 2] : v2[k], send = b4 ? v2[k] : v2[k + 2];
+        v3[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    v4 = (b2 ? v3[1] : v3[0]) + __shfl_xor_sync(0xffffffffu, b2 ? v3[0] : v3[1], 2);
+    v4 += __shfl_xor_sync(0xffffffffu, v4, 1);
+    const int q = (b8 ? 3 : 0) + (b4 ? 2 : 0) + (b2 ? 1 : 0);
+    owner = !(lane & 1) && q < 5 && !(b8 && b4) && !(b4 && b2);
+    col = (b16 ? 5 : 0) + q;
+}
+
 __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c, float (&s)[NSTAT])
 {
     __shared__ float sred[MAX_THREADS / 32][NSTAT];
     __shared__ float srow[MAX_THREADS][NSTAT + 1];
     const int TX = blockDim.x, tx = threadIdx.x, ty = threadIdx.y;
     const int lin = ty * TX + tx, warp = lin >> 5, lane = lin & 31;
-    const long long pstride = (long long)p.nz * p.nchunk;
-    float *out = p.partial + ((long long)c.y * NSTAT) * pstride + (long long)c.z * p.nchunk + c.chunk;
+    const long long pstride = (long long)p.nz * p.pchunks;
+    float *out = p.partial + ((long long)c.y * NSTAT) * pstride + (long long)c.z * p.pchunks + c.chunk;
     if ((TX & 31) == 0) {
-        // every warp lies inside one row segment: recursive-halving butterfly, 12 shuffles for
-        // the 10 sums (split 5|5, 3|3, 2|2, 1|1, then a plain exchange).  Afterwards the lanes
-        // 0, 2, 4, 8, 10 hold columns 0..4 and lanes 16, 18, 20, 24, 26 columns 5..9.
-        const bool b16 = lane & 16, b8 = lane & 8, b4 = lane & 4, b2 = lane & 2;
-        float v1[6], v2[4], v3[2];
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const float keep = b16 ? s[k + 5] : s[k], send = b16 ? s[k] : s[k + 5];
-            v1[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-        }
-        v1[5] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const float keep = b8 ? v1[k + 3] : v1[k], send = b8 ? v1[k] : v1[k + 3];
-            v2[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        }
-        v2[3] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const float keep = b4 ? v2[k + 2] : v2[k], send = b4 ? v2[k] : v2[k + 2];
-            v3[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-        }
-        float v4 = (b2 ? v3[1] : v3[0]) + __shfl_xor_sync(0xffffffffu, b2 ? v3[0] : v3[1], 2);
-        v4 += __shfl_xor_sync(0xffffffffu, v4, 1);
-        const int q = (b8 ? 3 : 0) + (b4 ? 2 : 0) + (b2 ? 1 : 0);
-        const bool owner = !(lane & 1) && q < 5 && !(b8 && b4) && !(b4 && b2);
-        const int col = (b16 ? 5 : 0) + q;
+        // every warp lies inside one row segment
+        float v4;
+        bool owner;
+        int col;
+        stats_warp_butterfly(s, lane, v4, owner, col);
         const int wpr = TX >> 5;
         if (wpr == 1) {
             if (owner) out[(long long)col * pstride] = v4;
@@ -726,6 +766,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
         if (geom) solid_fix_loads<V, RM>(p, c, g, S);
     }
     const float cda = __ldg(p.cda + c.y);
+    const float jr = __ldg(p.jref + c.y);
     float s[NSTAT];
     if constexpr (STATS) {
 #pragma unroll
@@ -733,13 +774,14 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
     }
 #pragma unroll
     for (int k = 0; k < V; ++k) {
-        const Cell m = moments<V>(p, g, k, cda);
+        mom_ref_shift<V>(g, k, jr);
+        const Cell m = moments<V>(p, g, k, cda, jr);
         if constexpr (STATS) {
             // solid cells are left out of the plane sums (the divisor stays nx*nz, as in the
             // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
             if (!MASK || !((solid_self<V>(S) >> k) & 1u)) stats_add(s, m);
         }
-        collide<V>(p, g, k, m);
+        collide<V>(p, g, k, m, jr);
     }
     const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
     if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
@@ -774,12 +816,12 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
     float r[V], ux[V], uy[V], uz[V];
 #pragma unroll
     for (int k = 0; k < V; ++k) {
-        const Cell m = moments<V>(p, g, k, cda);
+        const Cell m = moments<V>(p, g, k, cda, 0.f);
         const bool solid = MASK && ((solid_self<V>(S) >> k) & 1u);
         if (!solid) stats_add(s, m);
         r[k] = solid ? 1.0f : m.rho;             // solid cells report the rest state
         ux[k] = solid ? 0.f : m.ux; uy[k] = solid ? 0.f : m.uy; uz[k] = solid ? 0.f : m.uz;
-        if (!isfinite(r[k]) && p.diverged) *p.diverged = 1;   // LBM_EDIVERGED sentinel
+        if (!isfinite(r[k]) && p.diverged && c.z >= p.zv0 && c.z < p.zv1) *p.diverged = 1;   // LBM_EDIVERGED sentinel
     }
     const long long off = (long long)(c.y + p.ny * (c.z - p.z0)) * p.nx + c.x0 + p.zoff;
     if (p.rho_out) stv<V>(p.rho_out + off, r);

@@ -530,6 +530,11 @@ def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
     want = a.get_state().cpu().numpy()
     b = gpu.Lbm.from_config(cfg, aa=aa)
     b.set_state(ck, t0)
+    # the momentum reference is part of a bit-exact checkpoint (it changes rounding only)
+    ref = a.get_reference_profile()
+    assert np.any(ref != 0) and np.abs(ref - 0.05 * ((np.arange(10) + 0.5) / 10) ** (1 / 7)).max() < 1e-6
+    b.set_reference_profile(ref)
+    assert np.array_equal(b.get_reference_profile(), ref)
     assert b.time == t0
     assert np.array_equal(b.get_state().cpu().numpy(), ck.cpu().numpy())
     b.step(5)
@@ -626,3 +631,52 @@ def test_chunked_host_transfers(orc, gpu, monkeypatch):
         rd, ud = g.get_macros()
         assert np.array_equal(rh, rd.cpu().numpy()) and np.array_equal(uh, ud.cpu().numpy())
         g.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# TMA data path (lbm_tma.cuh) against the per-thread path: same arithmetic => identical bits
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("rows", [1, 2, 4])
+@pytest.mark.parametrize("nx", [256, 768])
+@pytest.mark.parametrize("bottom,top", BCS + [(wl.BOUNCE_BACK, wl.FORCED_EQ)],
+                         ids=["wall-slip", "wall-wall", "periodic", "wall-lid"])
+def test_tma_path_is_bit_identical_to_the_per_thread_path(orc, gpu, aa, rows, nx, bottom, top):
+    import torch
+    cfg = wl.small(nx=nx, ny=8, nz=5, bottom=bottom, top=top)
+    if top == wl.FORCED_EQ:
+        cfg["U_top"] = (0.06, 0.0, 0.01)
+    a = gpu.Lbm.from_config(cfg, aa=aa)
+    b = gpu.Lbm.from_config(cfg, aa=aa)
+    a.set_tma(0)
+    b.set_tma(7, rows)
+    assert "tma" not in a.variant and f"tma7x{rows}" in b.variant
+    for g in (a, b):
+        g.init(cfg["seed"])
+        g.stats_accumulate(1)
+    for n in (1, 1, 2, 5):
+        a.step(n)
+        b.step(n)
+        torch.cuda.synchronize()
+        assert torch.equal(a.get_state(), b.get_state()), n
+    sa, na = a.stats_read()
+    sb, nb = b.stats_read()
+    assert na == nb == 9
+    _check_stats(sb, sa, cfg["u_bulk"])
+    # and against the oracle
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    o.step(9)
+    assert _state_err(o, b, _weights(orc)) <= 2e-7
+
+
+def test_tma_is_refused_where_it_cannot_run(gpu):
+    g = gpu.Lbm(64, 4, 4, 0.01, 0.1)
+    with pytest.raises(gpu.LbmError) as e:
+        g.set_tma(2)
+    assert e.value.code == gpu.LBM_EINVAL
+    g.set_tma(0)
+    g = gpu.Lbm(256, 6, 4, 0.01, 0.1)
+    with pytest.raises(gpu.LbmError):
+        g.set_tma(7, 4)                      # 4 rows do not divide ny = 6
+    g.set_tma(7, 2)
