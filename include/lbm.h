@@ -226,10 +226,11 @@ long long lbm_launch_count(const lbm_t *h);
  * before the first lbm_step.  LBM_EINVAL if the shape does not tile the lattice. */
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
 
-/* Data-movement path of the step kernel.  mode is a bit mask of the step kinds that stream through
- * the Tensor Memory Accelerator (lbm_tma.cuh: cp.async.bulk.tensor tile loads/stores whose box
- * coordinates carry the streaming shift) instead of per-thread 128-bit accesses: bit 0 the AA even
- * step, bit 1 the AA odd step, bit 2 the two-lattice pull step; 0 = none.  rows = y rows per
+/* Data-movement path of the step kernel.  mode is a bit mask of the step kinds whose stream-in goes
+ * through the Tensor Memory Accelerator (lbm_tma.cuh: cp.async.bulk.tensor tile loads whose box
+ * coordinates carry the link's row and slot, x shift taken in shared memory) instead of per-thread
+ * 128-bit loads: bit 0 the AA even step, bit 1 the AA odd step, bit 2 the two-lattice pull step;
+ * 0 = none.  rows = y rows per
  * 256-cell tile (1, 2 or 4, must divide ny; 0 = keep).  Both paths compute the same thing with the
  * same per-cell arithmetic.  Available with 4 cells per thread, nx % 256 == 0 and no solid mask
  * (LBM_EINVAL otherwise); the environment variable LBM_TMA="mode[,rows]" sets the default of new

@@ -54,6 +54,11 @@ def lib():
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_set_top_velocity.argtypes = [C.c_void_p, dp]
         L.orc_set_solid.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_set_forest_codes.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
+        L.orc_forest_code.restype = C.c_uint32
+        L.orc_forest_code.argtypes = [C.c_int, C.c_int, C.c_double]
+        L.orc_forest_code_lad.restype = C.c_double
+        L.orc_forest_code_lad.argtypes = [C.c_uint32, C.c_double]
         L.orc_set_macros.argtypes = [C.c_void_p, dp, dp]
         L.orc_init_field.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_uint64, dp, dp]
         L.orc_init.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_uint64]
@@ -142,6 +147,27 @@ def lad_profile(h: int, ny: int, LAI: float, eta_m: float = 0.7) -> np.ndarray:
     return out
 
 
+def forest_code(h: int, y: int, y_m: float) -> int:
+    return int(lib().orc_forest_code(int(h), int(y), float(y_m)))
+
+
+def forest_code_lad(code: int, a_fm: float) -> float:
+    return float(lib().orc_forest_code_lad(C.c_uint32(code), float(a_fm)))
+
+
+def forest_codes_from_spec(spec: dict, shape):
+    """(codes (nz, ny, nx) uint32, a_fm) from a workloads `forest_cells` spec: a list of blocks
+    {x: (x0, x1), z: (z0, z1), y0, h, y_m} (half-open cell ranges; y_m in cells, 0 = constant LAD)."""
+    nz, ny, nx = shape
+    codes = np.zeros(shape, dtype=np.uint32)
+    for b in spec["blocks"]:
+        (x0, x1), (z0, z1) = b["x"], b["z"]
+        for j in range(b["h"]):
+            if 0 <= b["y0"] + j < ny:
+                codes[z0:z1, b["y0"] + j, x0:x1] = forest_code(b["h"], j, b["y_m"])
+    return codes, float(spec["a_fm"])
+
+
 def lad_from_spec(forest, ny: int):
     """lad_profile table from a workloads forest spec (None / uniform / lalic)."""
     if forest is None:
@@ -187,6 +213,8 @@ class Oracle:
             o.set_top_velocity(cfg["U_top"])
         if cfg.get("solid") is not None:
             o.set_solid(cfg["solid"])
+        if cfg.get("forest_cells") is not None:
+            o.set_forest_codes(*forest_codes_from_spec(cfg["forest_cells"], o.shape))
         return o
 
     def init_from_config(self, cfg: dict):
@@ -226,11 +254,19 @@ class Oracle:
         lib().orc_set_top_velocity(self._h, _dp(U))
 
     def set_solid(self, mask):
+        """Install / replace / remove (None) the solid cells, keeping the flow."""
         if mask is None:
             lib().orc_set_solid(self._h, None)
         else:
             m = np.ascontiguousarray(mask, dtype=np.uint8).reshape(self.shape)
             lib().orc_set_solid(self._h, m.ctypes.data_as(C.c_void_p))
+
+    def set_forest_codes(self, codes, a_fm: float):
+        if codes is None:
+            lib().orc_set_forest_codes(self._h, None, 0.0)
+        else:
+            c = np.ascontiguousarray(codes, dtype=np.uint32).reshape(self.shape)
+            lib().orc_set_forest_codes(self._h, c.ctypes.data_as(C.c_void_p), float(a_fm))
 
     def get_populations(self):
         f = np.zeros((19,) + self.shape)

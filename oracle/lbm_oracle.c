@@ -65,6 +65,8 @@ typedef struct orc_s {
     unsigned bc;
     double Utop[3];       /* forced-equilibrium lid velocity (NEXT #1) */
     unsigned char *solid; /* [N] 1 = solid (NEXT #2), NULL = none */
+    uint32_t *fcode;      /* [N] per-cell forest code (NEXT #2), NULL = none; 0 = use lad[y] */
+    double a_fm;          /* a_fm of Eq. 14 for the coded cells */
     double *fa, *fb;      /* [Q][N] */
     double *acc;          /* [ny][NSTAT] running sums */
     double *rowsum;       /* [nz][ny][NSTAT] scratch */
@@ -190,12 +192,48 @@ orc_t *orc_create(int nx, int ny, int nz, double nu, double Cs, const double *bo
 void orc_destroy(orc_t *o)
 {
     if (!o) return;
-    free(o->lad); free(o->solid); free(o->fa); free(o->fb); free(o->acc); free(o->rowsum);
+    free(o->lad); free(o->solid); free(o->fcode); free(o->fa); free(o->fb); free(o->acc); free(o->rowsum);
     free(o);
 }
 
 void orc_set_top_velocity(orc_t *o, const double *U) { for (int a = 0; a < 3; ++a) o->Utop[a] = U[a]; }
 
+/* Per-cell forest code: "The code for each forest cell contains ... h: height
+ * of the forest ...; y: distance in the vertical direction between the lower bounding box of the
+ * forest object and the current cell; y_m: distance ... between the lower bounding box of the
+ * forest and the maximum value of the LAD distribution.  This information is stored into the
+ * forest cell's code using a bit mask".  Layout chosen here (the paper gives none; DESIGN.md
+ * reading R27): bits 0-9 y (cells), bits 10-19 h (cells, 0 = not a forest cell), bits 20-31 y_m in
+ * eighths of a cell (0 = no maximum: constant LAD a_fm, Table II case 1).
+ * LAD of a coded cell, Eq. 14 (L107) with Eq. 15 (L112) at the cell centre eta = (y + 1/2)/h,
+ * eta_m = y_m/h: a_f = a_fm * shape(eta, eta_m). */
+uint32_t orc_forest_code(int h, int y, double y_m)
+{
+    uint32_t ym8 = (uint32_t)floor(y_m * 8.0 + 0.5);
+    return ((uint32_t)y & 1023u) | (((uint32_t)h & 1023u) << 10) | ((ym8 & 4095u) << 20);
+}
+double orc_forest_code_lad(uint32_t code, double a_fm)
+{
+    int y = (int)(code & 1023u), h = (int)((code >> 10) & 1023u);
+    double y_m = (double)((code >> 20) & 4095u) / 8.0;
+    if (h == 0 || y >= h) return 0.0;
+    if (y_m == 0.0) return a_fm;
+    return a_fm * orc_lad_shape((y + 0.5) / h, y_m / h);
+}
+void orc_set_forest_codes(orc_t *o, const uint32_t *code /* [N] or NULL */, double a_fm)
+{
+    free(o->fcode); o->fcode = NULL; o->a_fm = a_fm;
+    if (code) {
+        o->fcode = (uint32_t *)malloc(sizeof(uint32_t) * o->N);
+        memcpy(o->fcode, code, sizeof(uint32_t) * o->N);
+    }
+}
+
+/* Install (or with NULL remove) the solid cells AT RUN TIME, keeping the flow (PAPER.md:L226:
+ * "Once the turbulence is developed, the boxes are removed from the computational domain.  The
+ * flow remains in the turbulent status afterwards").  Cells that stay fluid keep their
+ * populations; a cell that is solid carries the rest state f = w, so a cell that turns fluid
+ * starts from f_eq(1, 0) (reading R28). */
 void orc_set_solid(orc_t *o, const unsigned char *mask /* [N] or NULL */)
 {
     free(o->solid); o->solid = NULL;
@@ -299,7 +337,7 @@ static void stream_cell(const orc_t *o, int x, int y, int z, double *f)
 }
 
 /* O3-O5: moments, predictor velocity, forest drag, corrected velocity, total force. */
-static void macros_cell(const orc_t *o, int y, const double *f, double *rho_out, double *u,
+static void macros_cell(const orc_t *o, long long cell, int y, const double *f, double *rho_out, double *u,
                         double *F, double *Pi /* [xx,yy,zz,xy,yz,xz] or NULL */)
 {
     double rho = 0.0, m[3] = {0, 0, 0};
@@ -320,6 +358,8 @@ static void macros_cell(const orc_t *o, int y, const double *f, double *rho_out,
     for (int a = 0; a < 3; ++a) us[a] = (m[a] + 0.5 * o->Fb[a]) / rho;
     double Ff[3] = {0, 0, 0};
     double a_j = o->lad[y];
+    /* Alg. 1 "if forest cell": a coded cell takes its LAD from its own code (L129-135) */
+    if (o->fcode && o->fcode[cell]) a_j = orc_forest_code_lad(o->fcode[cell], o->a_fm);
     if (a_j > 0.0) {
         /* Alg. 1, Eq. 13: F_f = -C_D a_f(y) |u| u, no rho factor (R4);
          * streamwise component only (R5) unless the vector form is flagged. */
@@ -384,7 +424,7 @@ void orc_get_macros(const orc_t *o, double *rho /*[N]*/, double *u /*[3][N]*/)
                 double f[Q], r, uu[3], F[3];
                 if (o->solid && o->solid[cell]) { rho[cell] = 1.0; u[cell] = u[o->N + cell] = u[2 * o->N + cell] = 0.0; continue; }
                 stream_cell(o, x, y, z, f);
-                macros_cell(o, y, f, &r, uu, F, NULL);
+                macros_cell(o, cell, y, f, &r, uu, F, NULL);
                 rho[cell] = r;
                 u[cell] = uu[0]; u[o->N + cell] = uu[1]; u[2 * o->N + cell] = uu[2];
             }
@@ -413,7 +453,7 @@ static void step_once(orc_t *o)
                     continue;
                 }
                 stream_cell(o, x, y, z, f);              /* Stream */
-                macros_cell(o, y, f, &rho, u, F, Pi);    /* u, F_f, corrected u */
+                macros_cell(o, cell, y, f, &rho, u, F, Pi);    /* u, F_f, corrected u */
                 if (sample) {                            /* O10: time + x-z plane averaging (L200, L251) */
                     rs[0] += u[0]; rs[1] += u[1]; rs[2] += u[2];
                     rs[3] += u[0] * u[0]; rs[4] += u[1] * u[1]; rs[5] += u[2] * u[2];

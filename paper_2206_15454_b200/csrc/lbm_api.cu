@@ -143,7 +143,9 @@ static void graph_drop(lbm_s *h)
     h->gexec = nullptr;
 }
 
-constexpr int TMA_DEFAULT_MODE = 7;
+// measured on cfg5 (profiles/r02_README.md): the TMA stream-in is correct but 5-7 % slower than the
+// per-thread loads on the AA odd step, so it is opt-in (lbm_set_tma / LBM_TMA)
+constexpr int TMA_DEFAULT_MODE = 0;
 
 static void set_variant(lbm_s *h)
 {
@@ -542,31 +544,32 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
 }
 
 template <int RM, int WM, bool S, int R>
-static cudaError_t launch_tma_r(lbm_s *h, const KParams &p, const CUtensorMap &ms, const CUtensorMap &md)
+static cudaError_t launch_tma_r(lbm_s *h, const KParams &p0, const CUtensorMap &ms)
 {
     static bool attr_set = false;
-    const int smem = Q * R * TMA_BOX * 4;
+    const int smem = (Q * R * TMA_BOX + Q * R) * 4;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(step_tma_kernel<RM, WM, S, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    dim3 block(TMA_TX, R), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / R * (h->nx / TMA_BOX)));
-    step_tma_kernel<RM, WM, S, R><<<grid, block, smem, h->stream>>>(p, ms, md);
+    KParams p = p0;
+    p.nchunk = h->nx / TMA_BOX;                   // tiles per row (make_ctx decomposes blockIdx with it)
+    dim3 block(TMA_TX, R), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / R * p.nchunk));
+    step_tma_kernel<RM, WM, S, R><<<grid, block, smem, h->stream>>>(p, ms);
     h->launches++;
     return cudaGetLastError();
 }
 template <int RM, int WM, bool S>
 static cudaError_t launch_tma(lbm_s *h, const KParams &p)
 {
-    // the maps follow the src/dst roles of this step (two-lattice: they swap every step)
+    // the map of the array this step reads (two-lattice: the roles swap every step)
     const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
     const CUtensorMap &ms = swapped ? h->map_b : h->map_a;
-    const CUtensorMap &md = h->aa ? h->map_a : (swapped ? h->map_a : h->map_b);
     switch (h->tma_rows) {
-    case 4: return launch_tma_r<RM, WM, S, 4>(h, p, ms, md);
-    case 2: return launch_tma_r<RM, WM, S, 2>(h, p, ms, md);
-    default: return launch_tma_r<RM, WM, S, 1>(h, p, ms, md);
+    case 4: return launch_tma_r<RM, WM, S, 4>(h, p, ms);
+    case 2: return launch_tma_r<RM, WM, S, 2>(h, p, ms);
+    default: return launch_tma_r<RM, WM, S, 1>(h, p, ms);
     }
 }
 

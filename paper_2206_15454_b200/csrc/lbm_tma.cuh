@@ -1,29 +1,24 @@
-// lbm_tma.cuh — the fused step with the streaming done by the Tensor Memory Accelerator.
+// lbm_tma.cuh — the fused step with the stream-in done by the Tensor Memory Accelerator.
 //
-// Same time step as lbm::step_kernel (Algorithm 1; the per-cell arithmetic is
-// the same moments()/collide() code), different data movement.  In step_kernel every thread moves
-// its own 4 cells with 128-bit accesses and pays for the +-1 x shift of 10 of the 19 directions
-// (Eq. 1) with shuffles, per-lane selects and scalar edge accesses: 13.8 warp instructions per
-// cell on the AA odd step against 9.8 on the even one (profiles/r01_README.md).  Here a CTA owns a
-// tile of 256 x R cells (R consecutive y rows of one z plane) and
-//   1. 19 lanes of warp 0 (one per direction) issue `cp.async.bulk.tensor` loads of the tile's
-//      R row segments of "their" population from wherever the streaming step says they come from:
-//      the box start coordinate carries the shift (x0 - c_x, y - c_y, z - c_z, slot), so the
-//      misalignment is absorbed by the TMA unit and the data lands ALIGNED in shared memory;
-//      boundary links (bounce-back, free-slip, periodic y, z wrap) are only a different
-//      (slot, y, z) of the box; all loads complete on one mbarrier;
-//   2. every thread reads its 4 cells x 19 populations with 19 LDS.128, runs moments / drag /
-//      Smagorinsky / collision (+ fused statistics), writes the result back to the same shared
-//      memory words (19 STS.128);
-//   3. after fence.proxy.async + one block barrier the 19 lanes issue `cp.async.bulk.tensor`
-//      stores with the push coordinates (x0 + c_x, ...), commit, wait for the reads of shared
-//      memory to finish and the CTA retires.  Several CTAs per SM overlap these phases.
-// The periodic x wrap is the one thing a box cannot express (coordinate -1 / nx is out of bounds:
-// loads fill zeros, stores clip): the issuing lane fetches / writes that single element of an
-// edge tile with a plain scalar access.
+// Same time step as lbm::step_kernel (Algorithm 1; the per-cell arithmetic, the
+// stores and the statistics are the same code), different stream-in.  In step_kernel every thread
+// fetches its own 4 cells with 128-bit loads and pays for the +-1 x shift of 10 of the 19
+// directions (Eq. 1) with a 64-bit address computation, a shuffle, per-lane selects and a
+// scalar edge load per direction.  Here a CTA owns a tile of 256 x R cells (R consecutive y rows
+// of one z plane) and
+//   1. one lane of every warp issues `cp.async.bulk.tensor` loads of the tile's R row segments of
+//      its share of the 19 populations, from wherever the streaming step says they come from: the
+//      box coordinate (x0, y - c_y, z - c_z, slot) carries the row and slot of the link (neighbour
+//      row, bounce-back / free-slip slot, periodic wrap), all 19 x R boxes complete on one mbarrier;
+//   2. the x shift is taken when the tile is read back: a thread's vector of direction i is its own
+//      aligned LDS.128 with the element of the neighbouring thread (one LDS.32) shifted in; the one
+//      element beyond the tile edge (with the periodic x wrap) is fetched by a scalar load into a
+//      halo word.  (The TMA unit itself cannot take the shift: a box must start on a 16-byte
+//      boundary of global memory - x0 - 1 raises an illegal-instruction fault, measured.)
+//   3. moments / drag / Smagorinsky / collision, stores and fused statistics as in step_kernel.
+// Several CTAs per SM overlap the phases.
 //
-// Requirements: 4 cells per thread layout (nx % 256 == 0), R | ny, no solid mask.  Everything
-// else (AA even/odd, two-lattice pull, lid, slabs) goes through the same kernel.
+// Requirements: 4 cells per thread layout (nx % 256 == 0), R | ny, no solid mask.
 #pragma once
 #include <cuda.h>
 
@@ -94,10 +89,10 @@ __device__ __forceinline__ void fence_proxy_async_smem()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
-// Where direction i of row y comes from (S1) / goes to (S7): the rules of load_dir / store_dir.
+// Where direction i of row y comes from (S1): the rules of load_dir.
 struct Link {
     int slot, y, z;
-    bool shifted;   // x is shifted by -c_x (source) / +c_x (destination)
+    bool shifted;   // x is shifted by -c_x
 };
 
 template <int RM>
@@ -129,110 +124,91 @@ __device__ __forceinline__ Link tma_source(const KParams &p, int i, int y, int z
     return l;
 }
 
-template <int WM>
-__device__ __forceinline__ Link tma_dest(const KParams &p, int i, int y, int z)
-{
-    const int cy = TMA_CY[i], cz = TMA_CZ[i];
-    Link l;
-    if (WM != WR_PUSH) {
-        l.slot = (WM == WR_LOCAL) ? i : TMA_OPP[i]; l.y = y; l.z = z; l.shifted = false;
-        return l;
-    }
-    const bool isbot = (y == 0), istop = (y == p.ny - 1);
-    const bool bb = (cy == -1 && isbot && p.bot == BC_BOT_WALL) ||
-                    (cy == 1 && istop && (p.top == BC_TOP_WALL || p.top == BC_TOP_LID));
-    const bool fs = (cy == 1 && istop && p.top == BC_TOP_SLIP);
-    int yd = y + cy;
-    if (yd < 0) yd = p.ny - 1;
-    if (yd >= p.ny) yd = 0;
-    int zd = z + cz;
-    if (zd < 0) zd = p.nz - 1;
-    if (zd >= p.nz) zd = 0;
-    l.slot = bb ? TMA_OPP[i] : (fs ? TMA_MIR[i] : i);
-    l.y = (bb || fs) ? y : yd;
-    l.z = bb ? z : zd;
-    l.shifted = !bb;
-    return l;
-}
-
 template <int R> struct TmaOcc { static constexpr int minb = (R == 1) ? 8 : (R == 2 ? 4 : (R == 4 ? 2 : 1)); };
 
-// grid = (nx/256) * (planes*ny/R) blocks, x chunks of a row adjacent; block = (64, R).
-// Dynamic shared memory: Q*R*256 floats.
+// grid = (nx/256) * (planes*ny/R) blocks, x chunks of a row adjacent (p.nchunk = nx/256);
+// block = (64, R).  Dynamic shared memory: Q*R*256 floats (tile) + Q*R floats (halo words).
 template <int RM, int WM, bool STATS, int R>
 __global__ void __launch_bounds__(TMA_TX *R, TmaOcc<R>::minb)
-step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc, const __grid_constant__ CUtensorMap mdst)
+step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc)
 {
     extern __shared__ __align__(128) unsigned char tma_smem[];
     float *buf = reinterpret_cast<float *>(tma_smem);   // [Q][R][256]
+    float *halo = buf + Q * R * TMA_BOX;                 // [Q][R]
     __shared__ __align__(8) uint64_t bar;
-    __shared__ float sred[STATS ? 2 * R : 1][NSTAT];
 
+    const Ctx c = make_ctx<4>(p, p.z0 * p.ny);
     const int tx = threadIdx.x, ty = threadIdx.y, lin = ty * TMA_TX + tx;
-    const int nch = p.nx / TMA_BOX;
-    const int rb = blockIdx.x / nch, chunk = blockIdx.x - rb * nch;
-    const int x0t = chunk * TMA_BOX;
-    const int row0 = p.z0 * p.ny + rb * R;
-    const int z = row0 / p.ny, y0 = row0 - z * p.ny;
-    const bool edge0 = (x0t == 0), edge1 = (x0t + TMA_BOX == p.nx);
-    const bool xshift = (RM != RD_LOCAL) || (WM == WR_PUSH);
+    const int x0t = c.chunk * TMA_BOX;
+    const int y0 = c.y - ty;                             // R | ny: the tile's rows share z
 
     if (lin == 0) mbar_init(&bar, 1);
     __syncthreads();
 
-    // ---- S1: stream in.  Lane i of warp 0 moves direction i. ----
-    float wrapv[R];
-    if (lin < 32) {
-        if (lin == 0) mbar_arrive_expect_tx(&bar, (uint32_t)(Q * R * TMA_BOX * 4));
-        __syncwarp();
-        if (lin < Q) {
-            const int i = lin, cx = TMA_CX[i];
+    // ---- S1: stream in.  Lane 0 of warp w moves the directions w, w + NW, ... (TMA instructions
+    // take warp-uniform operands: one issuing lane per warp, all warps issue in parallel). ----
+    constexpr int NW = (TMA_TX * R) / 32;
+    const int warp = lin >> 5, lane = lin & 31;
+    if (lin == 0) mbar_arrive_expect_tx(&bar, (uint32_t)(Q * R * TMA_BOX * 4));
+    if (lane == 0) {
+        for (int i = warp; i < Q; i += NW) {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const Link s = tma_source<RM>(p, i, y0 + r, z);
-                const int sx = s.shifted ? cx : 0;
-                tma_load_box(buf + (i * R + r) * TMA_BOX, &msrc, x0t - sx, s.y, s.z, s.slot, &bar);
-                wrapv[r] = 0.f;
-                if (RM != RD_LOCAL) {
-                    const float *rowp = p.src + (long long)s.slot * p.N + (long long)(s.y + p.ny * s.z) * p.nx;
-                    if (sx == 1 && edge0) wrapv[r] = rowp[p.nx - 1];
-                    if (sx == -1 && edge1) wrapv[r] = rowp[0];
-                }
+                const Link s = tma_source<RM>(p, i, y0 + r, c.z);
+                tma_load_box(buf + (i * R + r) * TMA_BOX, &msrc, x0t, s.y, s.z, s.slot, &bar);
             }
         }
     }
-    const int y = y0 + ty;
-    const float cda = __ldg(p.cda + y);
-    const float jr = __ldg(p.jref + y);
-    mbar_wait(&bar, 0);
-    if (RM != RD_LOCAL && (edge0 || edge1)) {
-        // the element a box cannot reach: x = -1 / x = nx of the periodic row
-        if (lin < Q) {
-            const int i = lin, cx = TMA_CX[i];
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const Link s = tma_source<RM>(p, i, y0 + r, z);
-                if (s.shifted && cx == 1 && edge0) buf[(i * R + r) * TMA_BOX] = wrapv[r];
-                if (s.shifted && cx == -1 && edge1) buf[(i * R + r) * TMA_BOX + TMA_BOX - 1] = wrapv[r];
+    if (RM != RD_LOCAL) {
+        // the element beyond the tile edge of every shifted box (periodic x wrap included)
+        if (lin < Q * R) {
+            const int i = lin / R, r = lin - i * R, cx = TMA_CX[i];
+            const Link s = tma_source<RM>(p, i, y0 + r, c.z);
+            if (s.shifted && cx != 0) {
+                int xs = (cx == 1) ? x0t - 1 : x0t + TMA_BOX;
+                xs = (xs < 0) ? p.nx - 1 : (xs >= p.nx ? 0 : xs);
+                halo[lin] = p.src[(long long)s.slot * p.N + (long long)(s.y + p.ny * s.z) * p.nx + xs];
             }
         }
         __syncthreads();
     }
+    const float cda = __ldg(p.cda + c.y);
+    const float jr = __ldg(p.jref + c.y);
+    mbar_wait(&bar, 0);
 
-    // ---- S2-S6 on the thread's 4 cells ----
+    // ---- read the thread's 4 cells x 19 directions back, x shift applied ----
     float g[Q][4];
-    float *mine = buf + ty * TMA_BOX + 4 * tx;
+    const float *mine = buf + ty * TMA_BOX + 4 * tx;
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        const float4 t = *reinterpret_cast<const float4 *>(mine + i * R * TMA_BOX);
-        g[i][0] = t.x; g[i][1] = t.y; g[i][2] = t.z; g[i][3] = t.w;
-        if constexpr (Lat::cy[i] == -1) {
-            if (p.top == BC_TOP_LID && y == p.ny - 1) {
+        constexpr int cx = Lat::cx[i], cy = Lat::cy[i];
+        const float *row = mine + i * R * TMA_BOX;
+        const float4 t = *reinterpret_cast<const float4 *>(row);
+        if constexpr (RM == RD_LOCAL || cx == 0) {
+            g[i][0] = t.x; g[i][1] = t.y; g[i][2] = t.z; g[i][3] = t.w;
+        } else {
+            bool bb = false;                           // a bounce-back link reads the own cell: no shift
+            if constexpr (cy == 1) bb = c.bot_bb;
+            if constexpr (cy == -1) bb = c.top_bb;
+            if constexpr (cx == 1) {                   // need x0-1 .. x0+2
+                const float *nb = (tx == 0) ? halo + i * R + ty : row - 1;
+                const float l = *nb;
+                g[i][0] = bb ? t.x : l; g[i][1] = bb ? t.y : t.x; g[i][2] = bb ? t.z : t.y; g[i][3] = bb ? t.w : t.z;
+            } else {                                   // need x0+1 .. x0+4
+                const float *nb = (tx == TMA_TX - 1) ? halo + i * R + ty : row + 4;
+                const float rr = *nb;
+                g[i][0] = bb ? t.x : t.y; g[i][1] = bb ? t.y : t.z; g[i][2] = bb ? t.z : t.w; g[i][3] = bb ? t.w : rr;
+            }
+        }
+        if constexpr (cy == -1) {
+            if (c.top_lid) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) g[i][k] = p.lid[lid_index(i)];
             }
         }
     });
+
+    // ---- S2-S8 as in step_kernel ----
     float s[NSTAT];
     if constexpr (STATS) {
 #pragma unroll
@@ -245,51 +221,15 @@ step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc, const
         if constexpr (STATS) stats_add(s, m);
         collide<4>(p, g, k, m, jr);
     }
-    static_for<0, Q>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        *reinterpret_cast<float4 *>(mine + i * R * TMA_BOX) = make_float4(g[i][0], g[i][1], g[i][2], g[i][3]);
-    });
-    fence_proxy_async_smem();
-
-    // ---- S8: x-row sums of the statistics (two warps per row segment) ----
-    float v4 = 0.f;
-    bool owner = false;
-    int col = 0;
+    const Ctx c2 = (WM == WR_PUSH) ? make_ctx<4>(p, p.z0 * p.ny, true) : c;
+    store_all<4, WM, false>(p, c2, g);
     if constexpr (STATS) {
         if (p.shift) {
-            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + y);
+            const float4 sh = __ldg(reinterpret_cast<const float4 *>(p.shift) + c2.y);
             stats_recentre(s, 4.0f, sh.x, sh.y, sh.z);
         }
-        stats_warp_butterfly(s, lin & 31, v4, owner, col);
-        if (owner) sred[lin >> 5][col] = v4;
+        stats_row_reduce(p, c2, s);
     }
-    __syncthreads();
-
-    // ---- S7: stream out ----
-    if (lin < Q) {
-        const int i = lin, cx = TMA_CX[i];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const Link d = tma_dest<WM>(p, i, y0 + r, z);
-            const int sx = d.shifted ? cx : 0;
-            const float *srcp = buf + (i * R + r) * TMA_BOX;
-            tma_store_box(&mdst, x0t + sx, d.y, d.z, d.slot, srcp);
-            if (WM == WR_PUSH) {
-                float *rowp = p.dst + (long long)d.slot * p.N + (long long)(d.y + p.ny * d.z) * p.nx;
-                if (sx == 1 && edge1) rowp[0] = srcp[TMA_BOX - 1];
-                if (sx == -1 && edge0) rowp[p.nx - 1] = srcp[0];
-            }
-        }
-        tma_store_commit_and_wait_read();
-    }
-    if constexpr (STATS) {
-        if (tx < NSTAT) {
-            const long long pstride = (long long)p.nz * p.pchunks;
-            float *out = p.partial + ((long long)y * NSTAT + tx) * pstride + (long long)z * p.pchunks + chunk;
-            *out = sred[2 * ty][tx] + sred[2 * ty + 1][tx];
-        }
-    }
-    (void)xshift;
 }
 
 } // namespace lbm

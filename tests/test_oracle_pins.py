@@ -667,3 +667,112 @@ def test_p16_relaxation_of_a_known_pi_neq(orc, Cs):
             # the pin has teeth: tau0 instead of tau_t would miss by far more than the bound
             miss = np.abs((1 / tau0 - 1 / tau_t) * fneq).max()
             assert miss > 1e-6 * np.abs(fneq).max() > 1e-11
+
+
+# ------------------------------------------------------------------------------------------
+# P17: run-time removal of the solid cells, reading R28
+# ------------------------------------------------------------------------------------------
+
+def test_p17_removing_solids_keeps_the_flow(orc):
+    """"Once the turbulence is developed, the boxes are removed ... The flow remains in the
+    turbulent status afterwards" (L226).  The removal call must leave every cell that was fluid
+    bit for bit as it was, hand the freed cells over at rest (f = w), conserve the total mass from
+    then on, and the first streaming step after it must be the plain (P13) push streaming."""
+    c, w, opp, mir = orc.tables()
+    cfg = wl.small(12, 8, 6)
+    solid = np.zeros((6, 8, 12), bool)
+    solid[1:4, 0:3, 2:5] = True                    # a trip box on the ground
+    solid[4:6, 0:2, 10:12] = True
+    o = orc.Oracle(12, 8, 6, cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                   orc.lad_from_spec(cfg["forest"], 8), orc.bc_flags("bounce_back", "free_slip", solid=True))
+    o.init(0, 0.05, 0.05, 17)
+    o.set_solid(solid)
+    o.step(40)                                     # spin up around the boxes
+    before = o.get_populations()
+    assert np.abs(before[:, ~solid] - w[:, None]).max() > 1e-3     # a real flow
+    # partial removal first (one box goes, one stays), then everything
+    keep = solid.copy()
+    keep[1:4, 0:3, 2:5] = False
+    for new in (keep, None):
+        o.set_solid(new)
+        after = o.get_populations()
+        assert np.array_equal(after[:, ~solid], before[:, ~solid])          # untouched cells
+        assert np.array_equal(after[:, solid], np.broadcast_to(w[:, None], after[:, solid].shape))
+        newmask = np.zeros_like(solid) if new is None else new
+        assert np.array_equal(o.stream_only(),
+                              _push_stream_solid(after, c, opp, mir, "bounce_back", "free_slip", newmask))
+    m0 = o.get_populations().sum()
+    o.step(200)
+    assert abs(o.get_populations().sum() - m0) <= 1e-12 * m0
+    rho, u = o.get_macros()
+    assert np.abs(u[:, solid]).max() > 1e-4        # the flow has entered the freed cells
+
+
+# ------------------------------------------------------------------------------------------
+# P18: per-cell forest codes (PAPER.md:L129-135; Alg. 1 L152 "if forest cell"), reading R27
+# ------------------------------------------------------------------------------------------
+
+def test_p18_forest_code_fields_and_lad(orc):
+    """Packing (h, y, y_m) and the LAD of a coded cell: Eq. 14 (L107) with Eq. 15 (L112) evaluated
+    here in closed form; y_m = 0 is the constant-LAD forest of Table II case 1."""
+    for h, y, ym in [(7, 0, 4.9), (7, 6, 4.9), (16, 11, 11.2), (48, 20, 33.6), (1023, 1022, 500.0)]:
+        code = orc.forest_code(h, y, ym)
+        assert code & 1023 == y and (code >> 10) & 1023 == h and (code >> 20) == round(ym * 8)
+        eta, eta_m = (y + 0.5) / h, round(ym * 8) / 8 / h
+        r = (1 - eta_m) / (1 - eta)
+        n = 6.0 if eta < eta_m else 0.5
+        assert orc.forest_code_lad(code, 0.38) == pytest.approx(0.38 * r ** n * np.exp(n * (1 - r)), rel=1e-13)
+    assert orc.forest_code_lad(orc.forest_code(7, 3, 0.0), 0.215) == 0.215
+    assert orc.forest_code_lad(0, 0.38) == 0.0                          # not a forest cell
+    assert orc.forest_code_lad(orc.forest_code(7, 7, 4.9), 0.38) == 0.0  # above the canopy top
+
+
+def test_p18_homogeneous_codes_equal_the_row_table(orc):
+    """A forest coded cell by cell over the whole x-z extent is the same problem as the per-row
+    LAD table a_j = a_fm s(eta_j) (computed here): populations agree to rounding over 60 steps."""
+    nx, ny, nz, h, ym, a_fm = 10, 12, 6, 5, 3.5, 0.3
+    eta = (np.arange(h) + 0.5) / h
+    r = (1 - ym / h) / (1 - eta)
+    n = np.where(eta < ym / h, 6.0, 0.5)
+    lad = np.zeros(ny)
+    lad[:h] = a_fm * r ** n * np.exp(n * (1 - r))
+    bc = orc.bc_flags("bounce_back", "free_slip")
+    a = orc.Oracle(nx, ny, nz, 1e-3, 0.1, (2e-6, 0, 0), 0.15, lad, bc)
+    b = orc.Oracle(nx, ny, nz, 1e-3, 0.1, (2e-6, 0, 0), 0.15, None, bc)
+    codes, afm = orc.forest_codes_from_spec(
+        dict(a_fm=a_fm, blocks=[dict(x=(0, nx), z=(0, nz), y0=0, h=h, y_m=ym)]), (nz, ny, nx))
+    assert afm == a_fm and np.count_nonzero(codes) == nx * nz * h
+    b.set_forest_codes(codes, a_fm)
+    for o in (a, b):
+        o.init(0, 0.05, 0.05, 18)
+        o.step(60)
+    assert np.abs(a.get_populations() - b.get_populations()).max() <= 1e-15
+    assert np.abs(a.get_populations() - orc.Oracle(nx, ny, nz, 1e-3, 0.1).get_populations()).max() > 1e-3
+
+
+def test_p18_partial_forest_is_local(orc):
+    """The collision is local (Alg. 1): after ONE step from the same state, the cells
+    inside a forest that covers part of the x-z plane equal the run with the row table everywhere,
+    all other cells equal the run without forest."""
+    nx, ny, nz, h, a_fm = 12, 8, 6, 4, 0.4
+    lad = np.zeros(ny)
+    lad[:h] = a_fm                                   # constant LAD (y_m = 0)
+    bc = orc.bc_flags("bounce_back", "free_slip", drag_vector=True)
+    mk = lambda l: orc.Oracle(nx, ny, nz, 1e-3, 0.1, (2e-6, 0, 0), 0.15, l, bc)
+    everywhere, nowhere, part = mk(lad), mk(None), mk(None)
+    spec = dict(a_fm=a_fm, blocks=[dict(x=(3, 9), z=(1, 4), y0=0, h=h, y_m=0.0)])
+    codes, _ = orc.forest_codes_from_spec(spec, (nz, ny, nx))
+    part.set_forest_codes(codes, a_fm)
+    f = everywhere.get_populations() * (1 + 0.2 * np.random.default_rng(8).uniform(-1, 1, (19, nz, ny, nx)))
+    for o in (everywhere, nowhere, part):
+        o.set_populations(f)
+        o.step(1)
+    inside = codes != 0
+    fe, fn, fp = everywhere.get_populations(), nowhere.get_populations(), part.get_populations()
+    assert np.array_equal(fp[:, inside], fe[:, inside]) and np.array_equal(fp[:, ~inside], fn[:, ~inside])
+    assert np.abs(fe[:, inside] - fn[:, inside]).max() > 1e-6       # the drag is really felt
+    # removing the codes restores the forest-free run
+    part.set_forest_codes(None, 0.0)
+    part.set_populations(f)
+    part.step(1)
+    assert np.array_equal(part.get_populations(), fn)
