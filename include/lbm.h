@@ -58,7 +58,8 @@ typedef enum lbm_status {
 #define LBM_TOP_PERIODIC      (2u << 2)   /*           periodic in y (must pair with BOTTOM_PERIODIC) */
 #define LBM_TOP_FORCED_EQ     (3u << 2)   /*           forced-equilibrium lid, the paper's ABL top (L216) */
 #define LBM_DRAG_VECTOR       (1u << 4)   /* bit 4: 0 streamwise-only drag (paper, L98/L103), 1 vector */
-#define LBM_SOLID_MASK        (1u << 5)   /* bit 5: a per-cell solid bit mask will be given (lbm_set_solid) */
+#define LBM_SOLID_MASK        (1u << 5)   /* bit 5: per-cell geometry: solid bit mask (lbm_set_solid) and
+                                             forest codes (lbm_set_forest_codes)                            */
 #define LBM_STORAGE_AA        (1u << 6)   /* bit 6: 0 two-lattice pull, 1 single-array AA pattern     */
 #define LBM_Z_HALO            (1u << 7)   /* bit 7: z slab of a larger lattice: planes 0 and nz-1 are ghost
                                              planes filled by the halo calls, planes 1..nz-2 are updated
@@ -97,15 +98,32 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs,
  * LBM_EINVAL if the handle was not created with LBM_TOP_FORCED_EQ or a component is not finite. */
 int lbm_set_top_velocity(lbm_t *h, const double *U_top);
 
-/* Per-cell solid geometry (LBM_SOLID_MASK; "a bit mask" codes the cell kind,
- * L226 turbulence-trip boxes).  solid_host: host, [nz][ny][nx] bytes,
- * non-zero = solid; NULL = no solid cell.  The library packs it to 1 bit per cell (one 32-bit word
- * per 32 x cells, 0.125 B/cell) in the workspace.  A link between a fluid and a solid cell is a
- * halfway bounce-back link; solid cells keep the rest state, report rho = 1, u = 0 and are left out
- * of the plane sums (the divisor of the averages stays nx*nz).  Call after lbm_bind; the state
- * must be (re-)initialised afterwards (lbm_init / lbm_set_macros*), LBM_ESTATE from lbm_step
- * otherwise.  Needs nx % 32 == 0 (checked at lbm_create). */
+/* Per-cell geometry (handles created with LBM_SOLID_MASK; "a bit mask" codes the
+ * cell kind, L226 turbulence-trip boxes).
+ *
+ * lbm_set_solid: solid_host is host, [nz][ny][nx] bytes, non-zero = solid; NULL = no solid cell.
+ * The library packs it to 1 bit per cell (one 32-bit word per 32 x cells, rows padded to whole
+ * words, 0.125 B/cell) in the workspace.  A link between a fluid and a solid cell is a halfway
+ * bounce-back link; solid cells keep the rest state, report rho = 1, u = 0 and are left out of the
+ * plane sums (the divisor of the averages stays nx*nz).  Call after lbm_bind, before or AFTER the
+ * state exists: on a running handle the flow is kept (L226: "the boxes are removed from the
+ * computational domain.  The flow remains in the turbulent status afterwards") - every cell that
+ * stays fluid keeps its populations bit for bit, a cell that turns fluid starts at rest
+ * (f = f_eq(1, 0), reading R28), a cell that turns solid is cleared; lbm_time is unchanged.
+ * Synchronises the stream.
+ *
+ * lbm_set_forest_codes: heterogeneous canopies (L129-135: "The code for each forest cell contains
+ * ... h ... y ... y_m ... stored into the forest cell's code using a bit mask"; Alg. 1 "if
+ * forest cell").  code_host is host, [nz][ny][nx] uint32, 0 = not a coded cell (the cell then uses
+ * lad_profile[y] of lbm_create), else lbm_forest_code(h, y, y_m): bits 0-9 y = cells above the
+ * forest base, bits 10-19 h = forest height in cells, bits 20-31 y_m = height of the LAD maximum in
+ * eighths of a cell (0 = constant LAD).  The cell's LAD is a_fm * shape((y+1/2)/h, y_m/h) of
+ * Eqs. 14-15 (a_fm when y_m = 0).  At most 255 distinct codes; the device keeps one byte per cell
+ * (read only in rows that hold coded cells) and a table of C_D a_f.  NULL removes the codes.
+ * LBM_EINVAL without LBM_SOLID_MASK.  Call after lbm_bind, at any time; synchronises the stream. */
 int lbm_set_solid(lbm_t *h, const uint8_t *solid_host);
+int lbm_set_forest_codes(lbm_t *h, const uint32_t *code_host, double a_fm);
+uint32_t lbm_forest_code(int h, int y, double y_m);
 
 /* Attach the caller-owned device workspace and stream; uploads the per-row tables.
  * Errors: LBM_ENOMEM (bytes < lbm_workspace_bytes or pointer not 256-B aligned), LBM_ECUDA. */

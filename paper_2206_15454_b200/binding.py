@@ -42,6 +42,7 @@ SYMBOLS = [
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
     "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma",
+    "lbm_set_forest_codes", "lbm_forest_code",
 ]
 
 
@@ -68,6 +69,9 @@ def lib():
         L.lbm_set_init.argtypes = [vp, C.c_int, C.c_double, C.c_double]
         L.lbm_set_top_velocity.argtypes = [vp, dp]
         L.lbm_set_solid.argtypes = [vp, C.c_void_p]
+        L.lbm_set_forest_codes.argtypes = [vp, C.c_void_p, C.c_double]
+        L.lbm_forest_code.argtypes = [C.c_int, C.c_int, C.c_double]
+        L.lbm_forest_code.restype = C.c_uint32
         L.lbm_set_graphs.argtypes = [vp, C.c_int]
         L.lbm_set_z_slab.argtypes = [vp, C.c_int, C.c_int]
         L.lbm_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
@@ -180,6 +184,23 @@ def mix64(seed: int, ctr: int) -> int:
     return int(lib().lbm_mix64(C.c_uint64(seed), C.c_uint64(ctr)))
 
 
+def forest_code(h: int, y: int, y_m: float) -> int:
+    return int(lib().lbm_forest_code(int(h), int(y), float(y_m)))
+
+
+def forest_codes_from_spec(spec: dict, shape):
+    """(codes (nz, ny, nx) uint32, a_fm) from a workloads `forest_cells` spec: a list of blocks
+    {x: (x0, x1), z: (z0, z1), y0, h, y_m} (half-open cell ranges; y_m in cells, 0 = constant LAD)."""
+    nz, ny, nx = shape
+    codes = np.zeros(shape, dtype=np.uint32)
+    for b in spec["blocks"]:
+        (x0, x1), (z0, z1) = b["x"], b["z"]
+        for j in range(b["h"]):
+            if 0 <= b["y0"] + j < ny:
+                codes[z0:z1, b["y0"] + j, x0:x1] = forest_code(b["h"], j, b["y_m"])
+    return codes, float(spec["a_fm"])
+
+
 def lad_from_spec(forest, ny: int):
     """lad_profile table from a workloads forest spec (None / uniform / lalic)."""
     if forest is None:
@@ -232,7 +253,8 @@ class Lbm:
         if aa is None:
             aa = cfg.get("storage", "two_lattice") == "aa"
         flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec,
-                         solid=cfg.get("solid") is not None, halo=halo)
+                         solid=cfg.get("solid") is not None or cfg.get("forest_cells") is not None
+                         or cfg.get("geometry", False), halo=halo)
         s = cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
                 lad_from_spec(cfg["forest"], cfg["ny"]), flags, **kw)
         i = cfg["init"]
@@ -241,6 +263,8 @@ class Lbm:
             s.set_top_velocity(cfg["U_top"])
         if cfg.get("solid") is not None:
             s.set_solid(cfg["solid"])
+        if cfg.get("forest_cells") is not None:
+            s.set_forest_codes(*forest_codes_from_spec(cfg["forest_cells"], s.shape))
         return s
 
     def close(self):
@@ -275,8 +299,19 @@ class Lbm:
     def set_launch_shape(self, tx: int, ty: int):
         _check(lib().lbm_set_launch_shape(self._h, int(tx), int(ty)))
 
+    def set_forest_codes(self, codes, a_fm: float = 0.0):
+        """codes: (nz, ny, nx) uint32 array of lbm_forest_code values (0 = none); None removes them."""
+        if codes is None:
+            _check(lib().lbm_set_forest_codes(self._h, None, 0.0))
+            return
+        c = np.ascontiguousarray(codes, dtype=np.uint32)
+        if c.shape != self.shape:
+            raise ValueError(f"forest codes must have shape {self.shape}")
+        _check(lib().lbm_set_forest_codes(self._h, C.c_void_p(c.ctypes.data), float(a_fm)))
+
     def set_solid(self, mask):
-        """mask: (nz, ny, nx) array, non-zero = solid; None clears.  Re-initialise afterwards."""
+        """mask: (nz, ny, nx) array, non-zero = solid; None clears.  On a running handle the flow
+        is kept (cells that turn fluid start at rest)."""
         if mask is None:
             _check(lib().lbm_set_solid(self._h, None))
             return

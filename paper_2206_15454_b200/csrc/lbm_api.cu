@@ -50,7 +50,7 @@ static size_t staging_budget()
 }
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, fidx, ftab, frow, staging, total;
     int stage_planes;
 };
 
@@ -71,6 +71,9 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     L.flag = off; off += 256;
     L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     L.solid_nb = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
+    L.fidx = off; if (mask) off = align_up(off + N, 256);              // per-cell forest table index, 1 B/cell
+    L.ftab = off; if (mask) off = align_up(off + 256 * 4, 256);
+    L.frow = off; if (mask) off = align_up(off + (size_t)ny, 256);
     const size_t plane = (size_t)16 * nx * ny;
     size_t planes = staging_budget() / plane;
     if (planes < 1) planes = 1;
@@ -90,6 +93,7 @@ struct lbm_s {
     int bot, top;
     bool aa, drag_vector, mask, halo;
     bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
+    bool forest_codes;          // per-cell forest codes installed (geometry handles)
     int zg0, nzg;               // z slab: global plane of local plane 0, global nz
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
     std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
@@ -237,8 +241,6 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
         return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
     int bot, top;
     if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
-    if ((bc_flags & LBM_SOLID_MASK) && nx % 32)
-        return fail(LBM_EINVAL, "LBM_SOLID_MASK needs nx %% 32 == 0 (got nx=%d)", nx);
     if (bc_flags & LBM_Z_HALO) {
         if (bc_flags & LBM_STORAGE_AA) return fail(LBM_EINVAL, "LBM_Z_HALO needs two-lattice storage");
         if (nz < 3) return fail(LBM_EINVAL, "LBM_Z_HALO needs nz >= 3 (two ghost planes + >= 1 interior)");
@@ -300,6 +302,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->graph_mode = 2; h->gexec = nullptr; h->g_steps = 0; h->g_parity = 0; h->g_every = 0;
     h->g_launches = 0; h->g_samples = 0;
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
+    h->forest_codes = false;
     set_variant(h);
     *out = h;
     return LBM_OK;
@@ -349,6 +352,9 @@ static void fill_params(lbm_s *h)
     p.solid = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid) : nullptr;
     p.solid_nb = h->mask ? reinterpret_cast<const unsigned *>(h->ws + h->L.solid_nb) : nullptr;
     p.nxw = (h->nx + 31) / 32;
+    p.fidx = (h->mask && h->forest_codes) ? reinterpret_cast<const unsigned char *>(h->ws + h->L.fidx) : nullptr;
+    p.ftab = h->mask ? reinterpret_cast<const float *>(h->ws + h->L.ftab) : nullptr;
+    p.frow = h->mask ? reinterpret_cast<const unsigned char *>(h->ws + h->L.frow) : nullptr;
     p.partial = nullptr; p.shift = nullptr;
     p.diverged = reinterpret_cast<int *>(h->ws + h->L.flag);
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
@@ -449,9 +455,12 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
             }
     // the mask dilated by one cell in every direction (periodic x, z; y only where periodic):
     // bit = some cell within one step is solid.  The kernels skip the geometry work where it is 0.
+    // A row is nxw words; the last one is ragged when nx % 32 != 0 (bits past nx stay 0).
     std::vector<uint32_t> nb;
     try { nb.assign(words, 0u); } catch (...) { return fail(LBM_ENOMEM, "host allocation failed"); }
     const bool yper = h->bot == BC_BOT_PERIODIC;
+    const int lastb = (h->nx - 1) & 31;
+    const uint32_t lastmask = (lastb == 31) ? 0xFFFFFFFFu : ((1u << (lastb + 1)) - 1u);
     for (int z = 0; z < h->nz; ++z)
         for (int y = 0; y < h->ny; ++y) {
             uint32_t *out = nb.data() + ((size_t)z * h->ny + y) * nxw;
@@ -462,15 +471,105 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
                     const int zz = (z + dz + h->nz) % h->nz;
                     const uint32_t *row = bits.data() + ((size_t)zz * h->ny + yy) * nxw;
                     for (int w = 0; w < nxw; ++w) {
-                        const uint32_t m = row[w], l = row[w == 0 ? nxw - 1 : w - 1], r = row[w + 1 == nxw ? 0 : w + 1];
-                        out[w] |= m | (m << 1) | (m >> 1) | (l >> 31) | (r << 31);
+                        const uint32_t m = row[w];
+                        // the bit left of this word's bit 0 and the bit right of its last valid bit
+                        const uint32_t lc = (w == 0) ? ((row[nxw - 1] >> lastb) & 1u) : (row[w - 1] >> 31);
+                        const uint32_t rc = (w + 1 == nxw) ? (row[0] & 1u) : (row[w + 1] & 1u);
+                        uint32_t v = m | (m << 1) | (m >> 1) | lc | (rc << ((w + 1 == nxw) ? lastb : 31));
+                        if (w + 1 == nxw) v &= lastmask;
+                        out[w] |= v;
                     }
                 }
         }
-    CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+    graph_drop(h);
+    if (h->inited) {
+        // run-time change: keep the flow.  The new mask waits in the staging area
+        // while the populations are moved from the old geometry's representation to the new one.
+        if (words * 4 > (size_t)(h->L.total - h->L.staging)) return fail(LBM_ENOMEM, "staging area too small for the mask");
+        uint32_t *newm = reinterpret_cast<uint32_t *>(h->ws + h->L.staging);
+        CU_TRY(cudaMemcpyAsync(newm, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+        KParams p = h->kp;
+        float *arr = (!h->aa && (h->t & 1)) ? p.dst : p.src;            // the array holding state t
+        const unsigned blocks = (unsigned)((h->N + 255) / 256);
+        if (h->aa && (h->t & 1) == 0)
+            mask_change_kernel<true><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
+        else
+            mask_change_kernel<false><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
+        h->launches++;
+        CU_TRY(cudaGetLastError());
+        CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, newm, words * 4, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+        CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+    }
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid_nb, nb.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaStreamSynchronize(h->stream));
-    h->inited = false;   // the populations must be rebuilt around the new geometry
+    return LBM_OK;
+}
+
+// Bit fields of a forest code (include/lbm.h): y | h << 10 | y_m (eighths of a cell) << 20.
+static double forest_code_lad(uint32_t code, double a_fm)
+{
+    const int y = (int)(code & 1023u), hc = (int)((code >> 10) & 1023u);
+    const double ym = (double)((code >> 20) & 4095u) / 8.0;
+    if (hc == 0 || y >= hc) return 0.0;
+    if (ym == 0.0) return a_fm;                              // constant LAD (Table II case 1)
+    // Eq. 14 (L107) with Eq. 15 (L112) at the cell centre
+    const double eta = (y + 0.5) / hc, eta_m = ym / hc;
+    const double ratio = (1.0 - eta_m) / (1.0 - eta);
+    const double n = (eta < eta_m) ? 6.0 : 0.5;
+    return a_fm * std::exp(n * std::log(ratio) + n * (1.0 - ratio));
+}
+
+uint32_t lbm_forest_code(int hc, int y, double y_m)
+{
+    const uint32_t ym8 = (uint32_t)std::floor(y_m * 8.0 + 0.5);
+    return ((uint32_t)y & 1023u) | (((uint32_t)hc & 1023u) << 10) | ((ym8 & 4095u) << 20);
+}
+
+int lbm_set_forest_codes(lbm_t *h, const uint32_t *code_host, double a_fm)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->mask) return fail(LBM_EINVAL, "per-cell forest codes need a geometry handle (LBM_SOLID_MASK)");
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_forest_codes before lbm_bind");
+    if (!(a_fm >= 0.0) || !std::isfinite(a_fm)) return fail(LBM_EINVAL, "a_fm must be >= 0");
+    graph_drop(h);
+    if (!code_host) {
+        h->forest_codes = false;
+        h->kp.fidx = nullptr;
+        return LBM_OK;
+    }
+    // distinct codes -> table of C_D a_f (fp32), one byte per cell indexes it
+    std::vector<uint8_t> idx;
+    std::vector<uint8_t> frow(h->ny, 0);
+    try { idx.assign((size_t)h->N, 0); } catch (...) { return fail(LBM_ENOMEM, "host allocation failed"); }
+    std::vector<uint32_t> codes;                             // codes[k-1] has table index k
+    std::vector<float> tab(256, 0.f);
+    uint32_t last = 0; int last_k = 0;
+    for (long long n = 0; n < h->N; ++n) {
+        const uint32_t c = code_host[n];
+        if (!c) continue;
+        int k = 0;
+        if (c == last) k = last_k;
+        else {
+            for (size_t q = 0; q < codes.size(); ++q) if (codes[q] == c) { k = (int)q + 1; break; }
+            if (!k) {
+                if (codes.size() >= 255) return fail(LBM_EINVAL, "more than 255 distinct forest codes");
+                codes.push_back(c);
+                k = (int)codes.size();
+                tab[k] = (float)(h->Cd * forest_code_lad(c, a_fm));
+            }
+            last = c; last_k = k;
+        }
+        idx[n] = (uint8_t)k;
+        frow[(n / h->nx) % h->ny] = 1;
+    }
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.fidx, idx.data(), (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.ftab, tab.data(), 256 * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.frow, frow.data(), (size_t)h->ny, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    h->forest_codes = true;
+    h->kp.fidx = reinterpret_cast<const unsigned char *>(h->ws + h->L.fidx);
     return LBM_OK;
 }
 

@@ -70,7 +70,10 @@ struct KParams {
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
     const unsigned *solid_nb;   // the same mask dilated by one cell in x, y, z (host-built)
-    int nxw;                    // words per x row (nx / 32)
+    int nxw;                    // words per x row, ceil(nx / 32) (bits past nx in the last word are 0)
+    const unsigned char *fidx;  // per-cell forest table index (0 = none), NULL = no coded forest
+    const float *ftab;          // [256] C_D * a_f of the forest codes in use
+    const unsigned char *frow;  // [ny] 1 = the row holds coded forest cells
     float lid[5];               // forced-equilibrium lid: f_eq,i(1, U_top) - w_i for i = 4, 8, 9, 16, 18
     // statistics
     float *partial;             // [ny][NSTAT][nz*nchunk]
@@ -320,10 +323,14 @@ __device__ __forceinline__ unsigned solid_field(const KParams &p, const Ctx &c, 
     const int w = c.x0 >> 5, b = c.x0 & 31;
     const unsigned m = __ldg(row + w);
     unsigned f = ((m >> b) & ((1u << V) - 1u)) << 1;
-    if (b > 0) f |= (m >> (b - 1)) & 1u;
-    else f |= __ldg(row + (w == 0 ? p.nxw - 1 : w - 1)) >> 31;
-    if (b + V < 32) f |= ((m >> (b + V)) & 1u) << (V + 1);
-    else f |= (__ldg(row + (w + 1 == p.nxw ? 0 : w + 1)) & 1u) << (V + 1);
+    // left neighbour x0-1 (periodic: x = nx-1 sits at bit (nx-1)&31 of the last word)
+    if (c.x0 == 0) f |= (__ldg(row + p.nxw - 1) >> ((p.nx - 1) & 31)) & 1u;
+    else if (b > 0) f |= (m >> (b - 1)) & 1u;
+    else f |= __ldg(row + w - 1) >> 31;
+    // right neighbour x0+V (periodic: x = 0)
+    if (c.x0 + V >= p.nx) f |= (__ldg(row) & 1u) << (V + 1);
+    else if (b + V < 32) f |= ((m >> (b + V)) & 1u) << (V + 1);
+    else f |= (__ldg(row + w + 1) & 1u) << (V + 1);
     return f;
 }
 
@@ -355,6 +362,33 @@ __device__ __forceinline__ unsigned solid_pick(unsigned long long S, int a, int 
 template <int V> __device__ __forceinline__ unsigned solid_self(unsigned long long S)
 {
     return (solid_pick(S, 1, 1) >> 1) & ((1u << V) - 1u);
+}
+
+// C_D a_f of the thread's cells: the row table, overridden cell by cell where a forest code is set
+// (Alg. 1 "if forest cell"; geometry handles only).  forest_idx fetches the
+// V table indices of the thread's cells packed in one word (0 = no coded cell in the row).
+template <int V, bool MASK>
+__device__ __forceinline__ unsigned forest_idx(const KParams &p, const Ctx &c)
+{
+    unsigned idx = 0u;
+    if constexpr (MASK) {
+        if (p.fidx && __ldg(p.frow + c.y)) {
+            const unsigned char *q = p.fidx + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0);
+            if constexpr (V == 4) idx = __ldg(reinterpret_cast<const unsigned *>(q));
+            else if constexpr (V == 2) idx = __ldg(reinterpret_cast<const unsigned short *>(q));
+            else idx = __ldg(q);
+        }
+    }
+    return idx;
+}
+template <bool MASK>
+__device__ __forceinline__ float cell_cda(const KParams &p, float row, unsigned idx, int k)
+{
+    if constexpr (MASK) {
+        const unsigned t = (idx >> (8 * k)) & 255u;
+        if (t) return __ldg(p.ftab + t);
+    }
+    return row;
 }
 
 template <int V, int RM>
@@ -744,9 +778,17 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
 // The step kernel.  grid = (row blocks, x chunks), block = (TX, TY) <= 256 threads.
 // ---------------------------------------------------------------------------------------------
 template <int V> struct Occ { static constexpr int minb = (V == 4) ? 2 : (V == 2 ? 3 : 4); };
+// (A larger register budget for the geometry variants - 168 registers, three blocks of 128
+// threads per SM - was measured and is slower than 128 registers with four blocks: 0.58 vs 0.47 ms
+// on cfg3 with statistics; profiles/r02_README.md.)
+constexpr int MASK_THREADS = 256;
+template <int V, bool MASK> struct Bounds {
+    static constexpr int threads = MAX_THREADS;
+    static constexpr int minb = Occ<V>::minb;
+};
 
 template <int V, int RM, int WM, bool STATS, bool MASK = false>
-__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const KParams p)
+__global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
     // With a mask, a warp none of whose lanes has a solid cell within one step (the usual case:
@@ -766,6 +808,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
         if (geom) solid_fix_loads<V, RM>(p, c, g, S);
     }
     const float cda = __ldg(p.cda + c.y);
+    const unsigned fidx = forest_idx<V, MASK>(p, c);
     const float jr = __ldg(p.jref + c.y);
     float s[NSTAT];
     if constexpr (STATS) {
@@ -775,7 +818,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
 #pragma unroll
     for (int k = 0; k < V; ++k) {
         mom_ref_shift<V>(g, k, jr);
-        const Cell m = moments<V>(p, g, k, cda, jr);
+        const Cell m = moments<V>(p, g, k, cell_cda<MASK>(p, cda, fidx, k), jr);
         if constexpr (STATS) {
             // solid cells are left out of the plane sums (the divisor stays nx*nz, as in the
             // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
@@ -799,7 +842,7 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) step_kernel(const K
 // rho/u when the pointers are given and the stage-1 sums when p.partial is given.
 // Covers rows [z0*ny, z1*ny).
 template <int V, int RM, bool MASK = false>
-__global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const KParams p)
+__global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) macros_kernel(const KParams p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
     float g[Q][V];
@@ -810,13 +853,14 @@ __global__ void __launch_bounds__(MAX_THREADS, Occ<V>::minb) macros_kernel(const
         if (__any_sync(0xffffffffu, S != 0ull)) solid_fix_loads<V, RM>(p, c, g, S);
     }
     const float cda = __ldg(p.cda + c.y);
+    const unsigned fidx = forest_idx<V, MASK>(p, c);
     float s[NSTAT];
 #pragma unroll
     for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
     float r[V], ux[V], uy[V], uz[V];
 #pragma unroll
     for (int k = 0; k < V; ++k) {
-        const Cell m = moments<V>(p, g, k, cda, 0.f);
+        const Cell m = moments<V>(p, g, k, cell_cda<MASK>(p, cda, fidx, k), 0.f);
         const bool solid = MASK && ((solid_self<V>(S) >> k) & 1u);
         if (!solid) stats_add(s, m);
         r[k] = solid ? 1.0f : m.rho;             // solid cells report the rest state
@@ -918,6 +962,78 @@ __device__ __forceinline__ bool solid_at(const KParams &p, int x, int y, int z)
 {
     if (!p.solid) return false;
     return (p.solid[(long long)(y + p.ny * z) * p.nxw + (x >> 5)] >> (x & 31)) & 1u;
+}
+
+// Where the AA "push" representation (t even) keeps population i of cell (x, y, z): slot and cell of
+// store_all<WR_PUSH> - the neighbour, or the own cell's opposite slot when the link bounces off a
+// wall face or a solid cell, or the mirrored slot of the tangential neighbour at a free-slip face.
+struct PushLoc { int slot; long long cell; bool self; };
+template <int i>
+__device__ __forceinline__ PushLoc push_target(const KParams &p, const unsigned *mask, int x, int y, int z)
+{
+    constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
+    const long long own = (long long)(y + p.ny * z) * p.nx + x;
+    int slot = i, xd = x + cx, yd = y + cy, zd = z + cz;
+    xd = (xd < 0) ? p.nx - 1 : (xd >= p.nx ? 0 : xd);
+    zd = (zd < 0) ? p.nz - 1 : (zd >= p.nz ? 0 : zd);
+    if (yd < 0) {
+        if (p.bot == BC_BOT_PERIODIC) yd = p.ny - 1;
+        else return {Lat::opp[i], own, true};
+    } else if (yd >= p.ny) {
+        if (p.top == BC_TOP_PERIODIC) yd = 0;
+        else if (p.top == BC_TOP_SLIP) { slot = Lat::mir[i]; yd = y; }
+        else return {Lat::opp[i], own, true};
+    }
+    if (mask && ((mask[(long long)(yd + p.ny * zd) * p.nxw + (xd >> 5)] >> (xd & 31)) & 1u)) return {Lat::opp[i], own, true};
+    return {slot, (long long)(yd + p.ny * zd) * p.nx + xd, false};
+}
+__device__ __forceinline__ bool mask_bit(const unsigned *mask, const KParams &p, long long cell)
+{
+    const long long row = cell / p.nx;
+    const int x = (int)(cell - row * p.nx);
+    return (mask[row * p.nxw + (x >> 5)] >> (x & 31)) & 1u;
+}
+
+// Run-time change of the solid mask that keeps the flow ("Once the turbulence is
+// developed, the boxes are removed ... The flow remains in the turbulent status afterwards").
+// One thread per cell; only cells whose bit changes act.  `arr` is the array holding state t.
+//   PUSH = false (two-lattice; AA at odd t): the representation does not depend on the mask; a cell
+//          that turns solid is cleared to the rest state, a cell that turns fluid holds it already.
+//   PUSH = true  (AA at even t): populations sit where the OLD mask sent them.  Between a changed
+//          cell d and a neighbour n that is fluid before and after:
+//            d turns fluid: n's population that had bounced off d (own slot of n) moves into d,
+//                           and n's slot receives d's rest population (0);
+//            d turns solid: n's population that had entered d bounces instead (moves to the own
+//                           slot of n, replacing what d had pushed there); d is cleared.
+template <bool PUSH>
+__global__ void mask_change_kernel(const KParams p, float *arr, const unsigned *oldm, const unsigned *newm)
+{
+    const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= p.N) return;
+    const bool was = mask_bit(oldm, p, d), is = mask_bit(newm, p, d);
+    if (was == is) return;
+    const int x = (int)(d % p.nx);
+    const long long row = d / p.nx;
+    const int y = (int)(row % p.ny), z = (int)(row / p.ny);
+    if constexpr (PUSH) {
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            // the link d --i--> n under the geometry in which d is fluid
+            const PushLoc t = push_target<i>(p, is ? oldm : newm, x, y, z);
+            if (t.self) return;
+            if (mask_bit(oldm, p, t.cell) || mask_bit(newm, p, t.cell)) return;   // n must be fluid before and after
+            float *at_n = arr + (long long)t.slot * p.N + t.cell;          // n's own slot on this link
+            float *at_d = arr + (long long)Lat::opp[i] * p.N + d;          // where n's population enters d
+            if (!is) { *at_d = *at_n; *at_n = 0.f; }                        // d turns fluid
+            else *at_n = *at_d;                                             // d turns solid
+        });
+    }
+    if (is) {
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            arr[(long long)i * p.N + d] = 0.f;
+        });
+    }
 }
 
 // Plain "state k" (post-collision, un-streamed) populations out of whatever representation the

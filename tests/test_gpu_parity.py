@@ -456,21 +456,99 @@ def test_solid_mask_parity(orc, gpu, aa, kind, nx, vec):
     assert np.all(rg.cpu().numpy()[solid] == 1.0) and np.all(ug.cpu().numpy()[:, solid] == 0.0)
 
 
-def test_solid_mask_needs_nx_multiple_of_32(gpu):
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("nx,vec", [(36, 4), (70, 2), (33, 1), (100, 4)])
+def test_solid_mask_on_ragged_rows(orc, gpu, aa, nx, vec):
+    """nx not a multiple of 32: the mask rows are padded to whole words (the paper's own meshes are
+    372, 350 and 250 cells wide)."""
+    cfg = wl.small(nx=nx, ny=8, nz=5)
+    m = np.random.default_rng(7).uniform(size=(5, 8, nx)) < 0.1
+    m[:, 0:2, nx - 2:] = True                  # a box across the x wrap
+    m[:, 0:2, :1] = True
+    cfg["solid"] = m
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    for n in (1, 2, 4):
+        o.step(n)
+        g.step(n)
+        assert _state_err(o, g, w) <= 2e-7
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("t_change", [6, 7])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2)])
+def test_solid_removed_at_run_time_keeps_the_flow(orc, gpu, aa, t_change, nx, vec):
+    """spin up around trip boxes, remove them, go on.  lbm_set_solid on a running
+    handle must agree with the oracle's run-time removal (pin P17) at both AA parities, for a
+    partial removal, a complete one and for boxes put back (cells turning solid)."""
+    cfg = wl.small(nx=nx, ny=10, nz=6)
+    boxes = _solid_mask("boxes", nx, 10, 6)
+    cfg["solid"] = boxes
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    o.step(t_change)
+    g.step(t_change)
+    part = boxes.copy()
+    part[1:4, 0:3, 5:9] = False                 # one box goes
+    moved = np.zeros_like(boxes)
+    moved[2:5, 3:6, 10:14] = True               # new solids in the middle of the flow, old ones gone
+    moved[0, 9, ::2] = True                     # and under the free-slip face
+    for mask, nsteps in ((part, 3), (None, 4), (moved, 3), (None, 20)):
+        o.set_solid(mask)
+        g.set_solid(mask)
+        assert g.time == o.time
+        assert _state_err(o, g, w) <= 2e-7      # the representation was converted, not re-initialised
+        o.step(nsteps)
+        g.step(nsteps)
+        assert _state_err(o, g, w) <= 3e-7
+        er, eu = _macro_err(o, g)
+        assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+    # the flow was kept: the freed cells carry momentum now
+    _, ug = g.get_macros()
+    assert float(ug[0].cpu().numpy()[boxes].std()) > 1e-4
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2), (33, 1)])
+def test_forest_codes_parity(orc, gpu, aa, nx, vec):
+    """Per-cell forest codes: a forest edge in x, a clearing in z, two canopy
+    heights and both LAD kinds (Eq. 14 and constant), next to a solid box."""
+    cfg = wl.small(nx=nx, ny=12, nz=6, forest_rows=0)
+    cfg["forest_cells"] = dict(a_fm=0.35, blocks=[
+        dict(x=(0, nx // 2), z=(0, 6), y0=0, h=5, y_m=3.5),
+        dict(x=(nx // 2 + 3, nx), z=(1, 4), y0=0, h=3, y_m=0.0),
+    ])
+    cfg["solid"] = np.zeros((6, 12, nx), bool)
+    cfg["solid"][2:4, 0:2, nx // 2:nx // 2 + 2] = True
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    o.stats_accumulate(1)
+    g.stats_accumulate(1)
+    for n in (1, 2, 6):
+        o.step(n)
+        g.step(n)
+        assert _state_err(o, g, w) <= 2e-7
+    er, eu = _macro_err(o, g)
+    assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+    _check_stats(g.stats_read()[0], o.stats_read()[0], cfg["u_bulk"])
+    # the codes matter (same run without them differs) and can be taken away again
+    o2 = orc.Oracle.from_config({**cfg, "forest_cells": None})
+    o2.init_from_config(cfg)
+    o2.step(9)
+    assert np.abs(o2.get_populations() - o.get_populations()).max() > 1e-6
+    g.set_forest_codes(None)
+    o.set_forest_codes(None, 0.0)
+    o.step(3)
+    g.step(3)
+    assert _state_err(o, g, w) <= 2e-7
+
+
+def test_forest_codes_need_a_geometry_handle(gpu):
+    g = gpu.Lbm(32, 4, 4, 0.01, 0.1)
     with pytest.raises(gpu.LbmError) as e:
-        gpu.Lbm(36, 4, 4, 0.01, 0.1, flags=gpu.bc_flags("bounce_back", "free_slip", solid=True))
+        g.set_forest_codes(np.zeros((4, 4, 32), np.uint32), 0.3)
     assert e.value.code == gpu.LBM_EINVAL
-
-
-def test_set_solid_requires_reinit(gpu):
-    g = gpu.Lbm(32, 4, 4, 0.01, 0.1, flags=gpu.bc_flags("bounce_back", "free_slip", solid=True))
-    g.set_init(gpu.INIT_REST, 0.0, 0.0)
-    g.init(1)
-    g.step(1)
-    g.set_solid(np.zeros((4, 4, 32), bool))
-    with pytest.raises(gpu.LbmError) as e:
-        g.step(1)
-    assert e.value.code == gpu.LBM_ESTATE
+    assert gpu.forest_code(7, 3, 4.9) == 0x2701C03
 
 
 # ---------------------------------------------------------------------------------------------
