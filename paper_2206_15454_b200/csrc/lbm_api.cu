@@ -50,7 +50,7 @@ static size_t staging_budget()
 }
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, fidx, ftab, frow, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, fidx, ftab, frow, bflag, staging, total;
     int stage_planes;
 };
 
@@ -74,6 +74,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     L.fidx = off; if (mask) off = align_up(off + N, 256);              // per-cell forest table index, 1 B/cell
     L.ftab = off; if (mask) off = align_up(off + 256 * 4, 256);
     L.frow = off; if (mask) off = align_up(off + (size_t)ny, 256);
+    L.bflag = off; if (mask) off = align_up(off + (size_t)ny * nz * MAX_NCHUNK, 256);   // one byte per thread block
     const size_t plane = (size_t)16 * nx * ny;
     size_t planes = staging_budget() / plane;
     if (planes < 1) planes = 1;
@@ -308,6 +309,8 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     return LBM_OK;
 }
 
+static int rebuild_block_flags(lbm_s *h);
+
 int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
@@ -321,7 +324,9 @@ int lbm_set_launch_shape(lbm_t *h, int tx, int ty)
     h->TX = tx; h->TY = ty; h->nchunk = W / tx;
     h->kp.nchunk = h->nchunk;
     set_variant(h);
-    return set_pchunks(h);
+    int rc = set_pchunks(h);
+    if (rc) return rc;
+    return rebuild_block_flags(h);
 }
 
 static void fill_params(lbm_s *h)
@@ -355,6 +360,7 @@ static void fill_params(lbm_s *h)
     p.fidx = (h->mask && h->forest_codes) ? reinterpret_cast<const unsigned char *>(h->ws + h->L.fidx) : nullptr;
     p.ftab = h->mask ? reinterpret_cast<const float *>(h->ws + h->L.ftab) : nullptr;
     p.frow = h->mask ? reinterpret_cast<const unsigned char *>(h->ws + h->L.frow) : nullptr;
+    p.bflag = h->mask ? reinterpret_cast<const unsigned char *>(h->ws + h->L.bflag) : nullptr;
     p.partial = nullptr; p.shift = nullptr;
     p.diverged = reinterpret_cast<int *>(h->ws + h->L.flag);
     p.uprof = reinterpret_cast<const float *>(h->ws + h->L.uprof);
@@ -425,9 +431,25 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
         const size_t mbytes = (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4;
         CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, mbytes, h->stream));
         CU_TRY(cudaMemsetAsync(h->ws + h->L.solid_nb, 0, mbytes, h->stream));
+        CU_TRY(cudaMemsetAsync(h->ws + h->L.bflag, 0, (size_t)h->ny * h->nz * MAX_NCHUNK, h->stream));
+        h->forest_codes = false;
+        h->kp.fidx = nullptr;
     }
     CU_TRY(cudaStreamSynchronize(h->stream)); // cda is a local vector
     h->bound = true; h->inited = false;
+    return LBM_OK;
+}
+
+// Rebuild the per-block geometry flags of the step launch (after a change of the mask, the forest
+// codes or the block shape).
+static int rebuild_block_flags(lbm_s *h)
+{
+    if (!h->mask || !h->bound) return LBM_OK;
+    const long long nblocks = (long long)h->ny * h->nz / h->TY * h->nchunk;
+    blockflag_kernel<<<(unsigned)((nblocks + 127) / 128), 128, 0, h->stream>>>(
+        h->kp, h->TX * h->V, h->TY, reinterpret_cast<unsigned char *>(h->ws + h->L.bflag), nblocks);
+    h->launches++;
+    CU_TRY(cudaGetLastError());
     return LBM_OK;
 }
 
@@ -502,6 +524,8 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
         CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid, bits.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
     }
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.solid_nb, nb.data(), words * 4, cudaMemcpyHostToDevice, h->stream));
+    int rc = rebuild_block_flags(h);
+    if (rc) return rc;
     CU_TRY(cudaStreamSynchronize(h->stream));
     return LBM_OK;
 }
@@ -537,6 +561,9 @@ int lbm_set_forest_codes(lbm_t *h, const uint32_t *code_host, double a_fm)
     if (!code_host) {
         h->forest_codes = false;
         h->kp.fidx = nullptr;
+        int rc0 = rebuild_block_flags(h);
+        if (rc0) return rc0;
+        CU_TRY(cudaStreamSynchronize(h->stream));
         return LBM_OK;
     }
     // distinct codes -> table of C_D a_f (fp32), one byte per cell indexes it
@@ -567,9 +594,11 @@ int lbm_set_forest_codes(lbm_t *h, const uint32_t *code_host, double a_fm)
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.fidx, idx.data(), (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.ftab, tab.data(), 256 * 4, cudaMemcpyHostToDevice, h->stream));
     CU_TRY(cudaMemcpyAsync(h->ws + h->L.frow, frow.data(), (size_t)h->ny, cudaMemcpyHostToDevice, h->stream));
-    CU_TRY(cudaStreamSynchronize(h->stream));
     h->forest_codes = true;
     h->kp.fidx = reinterpret_cast<const unsigned char *>(h->ws + h->L.fidx);
+    int rc = rebuild_block_flags(h);
+    if (rc) return rc;
+    CU_TRY(cudaStreamSynchronize(h->stream));
     return LBM_OK;
 }
 

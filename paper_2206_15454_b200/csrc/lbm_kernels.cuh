@@ -74,6 +74,8 @@ struct KParams {
     const unsigned char *fidx;  // per-cell forest table index (0 = none), NULL = no coded forest
     const float *ftab;          // [256] C_D * a_f of the forest codes in use
     const unsigned char *frow;  // [ny] 1 = the row holds coded forest cells
+    const unsigned char *bflag; // per thread block of the step launch: 1 = geometry (a solid cell within one
+                                // step of the block's cells, or a coded forest cell), 0 = plain fluid
     float lid[5];               // forced-equilibrium lid: f_eq,i(1, U_top) - w_i for i = 4, 8, 9, 16, 18
     // statistics
     float *partial;             // [ny][NSTAT][nz*nchunk]
@@ -787,8 +789,8 @@ template <int V, bool MASK> struct Bounds {
     static constexpr int minb = Occ<V>::minb;
 };
 
-template <int V, int RM, int WM, bool STATS, bool MASK = false>
-__global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
+template <int V, int RM, int WM, bool STATS, bool MASK>
+__device__ __forceinline__ void step_body(const KParams &p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
     // With a mask, a warp none of whose lanes has a solid cell within one step (the usual case:
@@ -836,6 +838,50 @@ __global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::min
         }
         stats_row_reduce(p, c2, s);
     }
+}
+
+// Geometry handles: a thread block none of whose cells has a solid cell within one step, nor a coded
+// forest cell, runs the plain body - the same code as the kernel without MASK (the per-block flag
+// is built by blockflag_kernel whenever the geometry or the block shape changes).  The flag is one
+// byte per block, read before anything else; in sparse geometry almost every block takes the plain
+// path, so the instruction cache sees one body.
+template <int V, int RM, int WM, bool STATS, bool MASK = false>
+__global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
+{
+    if constexpr (MASK) {
+        const long long gb = (long long)blockIdx.x + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
+        if (__ldg(p.bflag + gb) == 0) {
+            step_body<V, RM, WM, STATS, false>(p);
+            return;
+        }
+    }
+    step_body<V, RM, WM, STATS, MASK>(p);
+}
+
+// One thread per thread block of the step launch (block = tx_cells x ty rows, nchunk blocks per
+// row): flag = any bit of the dilated solid mask, or any coded forest cell, inside the block.
+__global__ void blockflag_kernel(const KParams p, int tx_cells, int ty, unsigned char *out, long long nblocks)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nblocks) return;
+    const long long rb = b / p.nchunk;
+    const int chunk = (int)(b - rb * p.nchunk);
+    const int x0 = chunk * tx_cells, x1 = x0 + tx_cells;
+    unsigned any = 0u;
+    for (int r = 0; r < ty; ++r) {
+        const long long row = rb * ty + r;
+        const unsigned *m = p.solid_nb + row * p.nxw;
+        for (int w = x0 >> 5; w <= (x1 - 1) >> 5; ++w) {
+            unsigned v = m[w];
+            const int lo = w << 5;
+            if (lo < x0) v &= ~0u << (x0 - lo);
+            if (lo + 32 > x1) v &= ~0u >> (lo + 32 - x1);
+            any |= v;
+        }
+        if (p.fidx && p.frow[row % p.ny])
+            for (int x = x0; x < x1; ++x) any |= p.fidx[row * p.nx + x];
+    }
+    out[b] = any ? 1 : 0;
 }
 
 // Sample S_k without changing the state (R19): the front half of the step (S1-S4).  Writes
