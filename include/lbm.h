@@ -274,6 +274,10 @@ const char *lbm_last_error(void);
  * a_j = LAI * s(eta_j) / sum_k s(eta_k) for j < h, 0 above, eta_j = (j+1/2)/h,
  * s(eta) = r^n exp[n(1-r)], r = (1-eta_m)/(1-eta), n = 6 (eta < eta_m) or 1/2. */
 int lbm_lad_profile(int h, int ny, double LAI, double eta_m, double *out_host);
+/* The same shape with the paper's own normalisation (Table II): a_j = a_fm * s(eta_j) for
+ * j < h (case 2: a_fm = 0.38 per metre, eta_m = 0.7), or the constant a_j = a_fm when eta_m = 0
+ * (case 1: 0.215 per metre); a_fm per lattice length. */
+int lbm_lad_eq14(int h, int ny, double a_fm, double eta_m, double *out_host);
 
 /* Host helpers (no CUDA) for the paper's normalised outputs, applied to
  * the [ny][LBM_NSTAT] table of lbm_stats_read.

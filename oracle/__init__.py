@@ -178,6 +178,11 @@ def lad_from_spec(forest, ny: int):
         return a
     if forest["kind"] == "lalic":
         return lad_profile(forest["h"], ny, forest["LAI"], forest.get("eta_m", 0.7))
+    if forest["kind"] == "eq14":       # the paper's own normalisation: a_j = a_fm s(eta_j) (Table II)
+        h, em = forest["h"], forest.get("eta_m", 0.7)
+        a = np.zeros(ny)
+        a[:h] = [forest["a_fm"] * (lad_shape((j + 0.5) / h, em) if em > 0 else 1.0) for j in range(h)]
+        return a
     raise ValueError(forest)
 
 

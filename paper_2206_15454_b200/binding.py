@@ -42,7 +42,7 @@ SYMBOLS = [
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
     "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma",
-    "lbm_set_forest_codes", "lbm_forest_code",
+    "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14",
 ]
 
 
@@ -109,6 +109,7 @@ def lib():
         L.lbm_destroy.restype = None
         L.lbm_last_error.restype = C.c_char_p
         L.lbm_lad_profile.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
+        L.lbm_lad_eq14.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
         L.lbm_set_kernel_timing.argtypes = [vp, C.c_int]
         L.lbm_kernel_timing_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.lbm_mix64.argtypes = [C.c_uint64, C.c_uint64]
@@ -138,6 +139,13 @@ def lad_profile(h: int, ny: int, LAI: float, eta_m: float = 0.7) -> np.ndarray:
     out = np.zeros(ny)
     _check(lib().lbm_lad_profile(int(h), int(ny), float(LAI), float(eta_m),
                                  out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
+def lad_eq14(h: int, ny: int, a_fm: float, eta_m: float = 0.7) -> np.ndarray:
+    out = np.zeros(ny)
+    _check(lib().lbm_lad_eq14(int(h), int(ny), float(a_fm), float(eta_m),
+                              out.ctypes.data_as(C.POINTER(C.c_double))))
     return out
 
 
@@ -211,6 +219,8 @@ def lad_from_spec(forest, ny: int):
         return a
     if forest["kind"] == "lalic":
         return lad_profile(forest["h"], ny, forest["LAI"], forest.get("eta_m", 0.7))
+    if forest["kind"] == "eq14":
+        return lad_eq14(forest["h"], ny, forest["a_fm"], forest.get("eta_m", 0.7))
     raise ValueError(forest)
 
 

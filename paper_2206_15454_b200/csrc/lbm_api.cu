@@ -1325,6 +1325,28 @@ int lbm_lad_profile(int hc, int ny, double LAI, double eta_m, double *out)
     return LBM_OK;
 }
 
+int lbm_lad_eq14(int hc, int ny, double a_fm, double eta_m, double *out)
+{
+    if (!out || ny < 1 || hc < 0 || hc > ny) return fail(LBM_EINVAL, "bad lad_eq14 arguments");
+    if (!(a_fm >= 0.0) || !std::isfinite(a_fm)) return fail(LBM_EINVAL, "a_fm must be >= 0");
+    if (!(eta_m >= 0.0 && eta_m < 1.0)) return fail(LBM_EINVAL, "eta_m must be in [0,1)");
+    for (int j = 0; j < ny; ++j) {
+        double a = 0.0;
+        if (j < hc) {
+            if (eta_m == 0.0) a = a_fm;               // constant LAD (Table II case 1)
+            else {
+                // Eq. 14 (L107) with Eq. 15 (L112), a_fm as printed (Table II case 2: 0.38 per metre)
+                const double eta = (j + 0.5) / hc;
+                const double ratio = (1.0 - eta_m) / (1.0 - eta);
+                const double n = (eta < eta_m) ? 6.0 : 0.5;
+                a = a_fm * std::exp(n * std::log(ratio) + n * (1.0 - ratio));
+            }
+        }
+        out[j] = a;
+    }
+    return LBM_OK;
+}
+
 int lbm_wall_friction_velocity(double F, double H, double rho, double *u_tau)
 {
     if (!u_tau) return fail(LBM_EINVAL, "u_tau is NULL");

@@ -67,8 +67,30 @@ CONFIGS = {
                  note="HBM-filling forest ABL, h=48, AA single array"),
 }
 
-# The paper's own lattice shapes.  Channel: Table I in lattice units
-# nu_lat = nu dt/dx^2 = 31^2/3250 * 1e-3, F_lat = F dt^2/dx; C_smag = 0.01.
+# The paper's own lattice shapes and cases.
+# Channel: Table I in lattice units, nu_lat = nu dt/dx^2 = 31^2/3250 * 1e-3, F_lat = F dt^2/dx
+# (PAPER.md:L185-192); C_smag = 0.01.
+# ABL: 1000 x 400 x 800 m, h = 20 m, no-slip ground, periodic x/z, forced-
+# equilibrium top moving with the free stream (L216), body force in the whole domain.  Table II:
+# case 1 a_f = 0.215 per metre (constant), case 2 Eq. 14 with z_m = 0.7 h and a_fm = 0.38 per metre,
+# case 3 no forest.  Table III meshes: 200x80x160, 250x100x200, 350x140x280 (dx = 5, 4, 20/7 m, so
+# h = 4, 5, 7 cells); LAD per lattice length = LAD per metre * dx.  The paper's body-force number is
+# garbled (L216, R22): F is the SURVEY.md §8(d) balance F (ny - h) = (U_top/12)^2.
+def abl_case(name, nx, ny, nz, h, case, note):
+    """One of the paper's ABL cases (Table II) on an nx x ny x nz mesh with a canopy of h cells."""
+    dx = 1000.0 / nx
+    forest = {1: dict(kind="eq14", h=h, a_fm=0.215 * dx, eta_m=0.0),
+              2: dict(kind="eq14", h=h, a_fm=0.38 * dx, eta_m=0.7),
+              3: None}[case]
+    U = 0.08
+    c = _cfg(name, nx, ny, nz, 1e-4, 0.1, (U / 12.0) ** 2 / (ny - h), 0.15, BOUNCE_BACK, FORCED_EQ, forest,
+             INIT_POWER_LAW, U, 0.05, u_bulk=U, steps=200, note=note)
+    c["U_top"] = (U, 0.0, 0.0)
+    c["h"] = h
+    c["case"] = case
+    return c
+
+
 PAPER_SIZED = {
     "paper_channel": _cfg("paper_channel", 372, 62, 124, 2.9569230769230769e-4, 0.1,
                           9.2566e-8, 0.0, BOUNCE_BACK, BOUNCE_BACK, None, INIT_PARABOLA,
@@ -77,8 +99,28 @@ PAPER_SIZED = {
     "paper_abl_fine": _cfg("paper_abl_fine", 350, 140, 280, 1e-4, 0.1, 1.0e-7, 0.15,
                            BOUNCE_BACK, FREE_SLIP, dict(kind="uniform", a=0.215 * 1000.0 / 350.0, rows=7),
                            INIT_POWER_LAW, 0.08, 0.05, u_bulk=0.08, steps=200,
-                           note="PAPER.md:L244 Table III fine mesh, Table II case 1 (a_f=0.215/m, h=7 cells)"),
+                           note="PAPER.md:L244 Table III fine mesh, Table II case 1 (a_f=0.215/m, h=7 cells), free-slip top"),
+    "paper_abl_fine_case1": abl_case("paper_abl_fine_case1", 350, 140, 280, 7, 1,
+                                 "Table III fine mesh, Table II case 1 (constant LAD 0.215/m), forced-equilibrium top"),
+    "paper_abl_fine_case2": abl_case("paper_abl_fine_case2", 350, 140, 280, 7, 2,
+                                 "Table III fine mesh, Table II case 2 (Eq. 14, z_m=0.7h, a_fm=0.38/m)"),
+    "paper_abl_fine_case3": abl_case("paper_abl_fine_case3", 350, 140, 280, 7, 3,
+                                 "Table III fine mesh, Table II case 3 (no forest)"),
+    "paper_abl_medium": abl_case("paper_abl_medium", 250, 100, 200, 5, 2, "Table III medium mesh 250x100x200, case 2"),
+    "paper_abl_coarse": abl_case("paper_abl_coarse", 200, 80, 160, 4, 2, "Table III coarse mesh 200x80x160, case 2"),
 }
+
+
+def abl_case_small(case: int, nx=48, ny=28, nz=24, h=7, seed=DEFAULT_SEED) -> dict:
+    """An oracle-sized ABL of the paper's structure (Table II case 1, 2 or 3; h = 7 cells as on the
+    fine mesh, dx of the fine mesh) for the qualitative checks of PAPER.md:L283-305."""
+    c = abl_case(f"abl_small_case{case}", nx, ny, nz, h, case, "oracle-sized Table II case")
+    dx = 1000.0 / 350.0
+    if c["forest"] is not None:
+        c["forest"]["a_fm"] = (0.215 if case == 1 else 0.38) * dx
+    c["nu"] = 1e-3
+    c["seed"] = seed
+    return c
 
 
 def get(name: str) -> dict:
