@@ -381,9 +381,10 @@ def run_b200(args, cfg):
 
 def run_sharded(args, cfg):
     """--sharded: ONE lattice of nx x ny x (N nz) cut into N z slabs (two-lattice storage), one
-    halo exchange per step over torch.distributed.  Opt-in: the default --gpus N
-    path stays N replicas, because this run's hardware has one GPU and the NCCL leg could only be
-    exercised with N = 1 (self exchange) and emulated rings."""
+    halo exchange per step over torch.distributed, overlapped with the interior update
+    (DESIGN.md "Multi-GPU").  Opt-in: north_star asks for one GPU, so the default --gpus N path
+    stays N replicas; on this run's hardware the NCCL leg could only be exercised with N = 1
+    (self exchange through the second stream) and emulated rings."""
     import numpy as np
     import torch
     import torch.distributed as dist
@@ -398,46 +399,100 @@ def run_sharded(args, cfg):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
     g = dict(cfg)
     g["nz"] = cfg["nz"] * world
     g["storage"] = "two_lattice"
     K, W = args.steps, args.warmup
     N = wl.n_cells(cfg)
+    every = cfg.get("stats_every", 0)
     s = slab.SlabLbm(g, rank, world, device=dev)
     s.init(cfg["seed"])
-    s.stats_accumulate(cfg.get("stats_every", 0))
+    s.stats_accumulate(every)
     s.step(W)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
+    barrier()
     sampler = ClockSampler(local)
     sampler.begin()
     stream = torch.cuda.current_stream(dev)
     l0 = s.sim.launch_count
+    same_pass = N * BYTES_PER_CELL / 6.5e12 > 1e-3 and 3 * K <= 4096
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if same_pass:
+        s.sim.set_kernel_timing(True)
     e0.record(stream)
     s.step(K)
     e1.record(stream)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    ms = max_over_ranks([e0.elapsed_time(e1)], world, dev)[0]
+    barrier()
+    ms = e0.elapsed_time(e1)
     launches = s.sim.launch_count - l0
     clocks = sampler.result()
     st = s.stats_read()
     if not np.isfinite(st).all():
         raise RuntimeError("sharded run produced non-finite statistics")
+    nk = K
+    if not same_pass:
+        nk = min(K, 1300)
+        s.sim.set_kernel_timing(True)
+        s.step(nk)
+    k_ms, _k_n = s.sim.kernel_timing_read()
+    s.sim.set_kernel_timing(False)
+    kernel_ms = k_ms / nk                      # boundary-plane + interior launches of one step
+
+    # end to end: host fields of the slab -> device, then K x [step + statistics read (all-reduce + D2H)]
+    rho_h = torch.empty(s.sim.shape, dtype=torch.float32).pin_memory()
+    u_h = torch.empty((3,) + s.sim.shape, dtype=torch.float32).pin_memory()
+    s.sim.get_macros_host(rho_h, u_h)
+    barrier()
+    t0 = time.perf_counter()
+    s.sim.set_macros_host(rho_h, u_h)
+    s.exchange()
+    s.stats_accumulate(max(1, every))
+    out = None
+    for _ in range(K):
+        s.step(1)
+        out = s.stats_read()
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    if not np.isfinite(out).all():
+        raise RuntimeError("end-to-end leg produced non-finite statistics")
+    ms, e2e_ms, kernel_ms = max_over_ranks([ms, e2e_ms, kernel_ms], world, dev)
+    variant = s.sim.variant
     if rank == 0:
+        peak, peak_src = measured_peak()
         mlups = aggregate_mlups(N, K, ms, world)
-        cfgd = workload_config(g, args, s.sim.variant)
-        cfgd["parallelism"] = f"one lattice in {world} z slab(s), ring halo exchange of 2 x 5 x nx x ny fp32 per step"
-        print(json.dumps({
+        achieved = BYTES_PER_CELL * N / (kernel_ms * 1e-3) / 1e9
+        cfgd = workload_config(g, args, variant)
+        cfgd["parallelism"] = (f"one lattice in {world} z slab(s), ring halo exchange of 2 x 5 x nx x ny fp32 "
+                               "per step on a second stream, overlapped with the interior update")
+        line = {
             "metric": METRIC, "value": round(mlups, 1), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": round(ms / K, 5), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfgd,
             "algorithmic_gbs": round(mlups * BYTES_PER_CELL / 1e3 / world, 1),
+            "frac_of_nominal_8tbs": round(mlups * BYTES_PER_CELL / 1e3 / world / 8000.0, 4),
+            "roofline": {"bound": "hbm", "kernel": "lbm::step_kernel (" + variant + "), boundary + interior launches",
+                         "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                         "frac": round(achieved / peak, 4), "traffic": None, "traffic_source": None,
+                         "peak_source": peak_src, "bytes_per_cell": BYTES_PER_CELL,
+                         "kernel_ms": round(kernel_ms, 5),
+                         "timed_in": "the K timed steps themselves" if same_pass else "a second pass"},
+            "e2e": {"value": round(aggregate_mlups(N, K, e2e_ms, world), 1), "unit": UNIT,
+                    "h2d_bytes_per_step": int((rho_h.numel() + u_h.numel()) * 4 / K),
+                    "d2h_bytes_per_step": int(cfg["ny"] * lb.NSTAT * 8 + 8), "steps": K,
+                    "what": "lbm_set_macros_host(pinned slab fields) + steps x [slab step + stats read (all-reduce)]"},
             "halo_bytes_per_step": 2 * 5 * cfg["nx"] * cfg["ny"] * 4,
-            "gpu_launches": int(launches), "clocks": clocks, "mode": "sharded"}))
+            "gpu_launches": int(launches), "clocks": clocks, "mode": "sharded"}
+        if not args.no_cpu and world == 1:
+            cm, _cms, _cs, cores, sample = time_oracle(cfg, 0, 1)
+            line["cpu_baseline"] = {"value": round(cm, 2), "unit": UNIT, "cores": cores,
+                                    "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    s.close()
     if world > 1:
         dist.destroy_process_group()
     return 0

@@ -178,6 +178,26 @@ int lbm_halo_bytes(const lbm_t *h, size_t *bytes);
 int lbm_halo_pack(lbm_t *h, int side, float *buf_dev);
 int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev);
 
+/* One time step of a z slab with the halo exchange overlapped by the interior update (what
+ * lbm_step(1) + pack + exchange + unpack do one after the other):
+ *   lbm_step_slab_begin  updates the two boundary planes (1 and nz-2), packs the faces of the new
+ *                        state into send_lo_dev / send_hi_dev ([5][ny][nx] fp32 each, as
+ *                        lbm_halo_pack side 0 / 1), records packed_event (a cudaEvent_t passed as
+ *                        void*, may be NULL) on the bound stream, then launches the update of the
+ *                        interior planes.  Asynchronous.
+ *   the caller           makes its communication stream wait for packed_event, sends send_hi to
+ *                        the upper and send_lo to the lower ring neighbour, receives the lower
+ *                        neighbour's high face into recv_lo and the upper neighbour's low face
+ *                        into recv_hi, and records ready_event there: the transfer runs while the
+ *                        interior planes are being updated.
+ *   lbm_step_slab_end    makes the bound stream wait for ready_event (NULL = no wait), unpacks the
+ *                        two buffers into the ghost planes of the new state, runs the statistics
+ *                        stage 2 of a sampled step and advances lbm_time.  Asynchronous.
+ * Results are bit-identical to the sequential form.  LBM_ESTATE if the calls do not alternate;
+ * LBM_EINVAL without LBM_Z_HALO. */
+int lbm_step_slab_begin(lbm_t *h, float *send_lo_dev, float *send_hi_dev, void *packed_event);
+int lbm_step_slab_end(lbm_t *h, const float *recv_lo_dev, const float *recv_hi_dev, void *ready_event);
+
 /* Raw running sums behind lbm_stats_read, for combining slabs: out_host [ny][LBM_NSTAT] doubles of
  * sum(u-u0), sum(v-v0), sum(w-w0), the six centred second-moment sums and sum(rho) over the
  * samples and cells seen so far (column 9 holds sum(rho)); centre_host [ny][3] doubles = (u0, v0, w0) per row (may be NULL);

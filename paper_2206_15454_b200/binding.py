@@ -42,7 +42,7 @@ SYMBOLS = [
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
     "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma",
-    "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14",
+    "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14", "lbm_step_slab_begin", "lbm_step_slab_end",
 ]
 
 
@@ -77,6 +77,8 @@ def lib():
         L.lbm_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
         L.lbm_halo_pack.argtypes = [vp, C.c_int, fp]
         L.lbm_halo_unpack.argtypes = [vp, C.c_int, fp]
+        L.lbm_step_slab_begin.argtypes = [vp, fp, fp, vp]
+        L.lbm_step_slab_end.argtypes = [vp, fp, fp, vp]
         L.lbm_stats_read_raw.argtypes = [vp, dp, dp, dp]
         L.lbm_stats_from_raw.argtypes = [dp, dp, C.c_int, C.c_double, dp]
         L.lbm_wall_friction_velocity.argtypes = [C.c_double, C.c_double, C.c_double, dp]
@@ -462,6 +464,18 @@ class Lbm:
 
     def halo_unpack(self, side: int, buf):
         _check(lib().lbm_halo_unpack(self._h, int(side), self._dev(buf, (5, self.ny, self.nx))))
+
+    def step_slab_begin(self, send_lo, send_hi, packed_event=None):
+        """Boundary planes, pack, record `packed_event` (a torch.cuda.Event), interior planes."""
+        ev = C.c_void_p(packed_event.cuda_event) if packed_event is not None else None
+        shp = (5, self.ny, self.nx)
+        _check(lib().lbm_step_slab_begin(self._h, self._dev(send_lo, shp), self._dev(send_hi, shp), ev))
+
+    def step_slab_end(self, recv_lo, recv_hi, ready_event=None):
+        """Wait for `ready_event`, unpack the ghost planes, finish the step."""
+        ev = C.c_void_p(ready_event.cuda_event) if ready_event is not None else None
+        shp = (5, self.ny, self.nx)
+        _check(lib().lbm_step_slab_end(self._h, self._dev(recv_lo, shp), self._dev(recv_hi, shp), ev))
 
     def stats_read_raw(self):
         """(raw sums [ny][10], centre [ny][3], count) - additive over slabs when the centre is 0."""

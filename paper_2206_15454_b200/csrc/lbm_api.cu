@@ -95,6 +95,7 @@ struct lbm_s {
     bool aa, drag_vector, mask, halo;
     bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
     bool forest_codes;          // per-cell forest codes installed (geometry handles)
+    bool slab_open, slab_sample; // between lbm_step_slab_begin and _end; that step samples
     int zg0, nzg;               // z slab: global plane of local plane 0, global nz
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
     std::vector<double> nfluid; // fluid cells per y plane (nx*nz without a mask)
@@ -304,6 +305,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->g_launches = 0; h->g_samples = 0;
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
     h->forest_codes = false;
+    h->slab_open = false; h->slab_sample = false;
     set_variant(h);
     *out = h;
     return LBM_OK;
@@ -879,32 +881,47 @@ int lbm_set_macros_host(lbm_t *h, const float *rho_host, const float *u_host)
     return LBM_OK;
 }
 
+// one step-kernel launch, bracketed by a pair of events when kernel timing is on
+static int launch_step_timed(lbm_s *h, const KParams &p, bool sample)
+{
+    const bool timed = h->timing && h->ev_used + 2 <= 2 * MAX_TIMED;
+    if (timed) {
+        while (h->ev.size() < h->ev_used + 2) {
+            cudaEvent_t e;
+            CU_TRY(cudaEventCreate(&e));
+            h->ev.push_back(e);
+        }
+        CU_TRY(cudaEventRecord(h->ev[h->ev_used], h->stream));
+    }
+    CU_TRY(launch_step(h, p, sample));
+    if (timed) {
+        CU_TRY(cudaEventRecord(h->ev[h->ev_used + 1], h->stream));
+        h->ev_used += 2;
+    }
+    return LBM_OK;
+}
+
+// parameters of the step that maps state t -> t+1
+static KParams step_params(lbm_s *h, bool sample)
+{
+    KParams p = h->kp;
+    if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
+    p.z0 = h->zlo; p.z1 = h->zhi;
+    if (sample) {
+        p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
+        p.shift = (h->mask || h->halo) ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
+    }
+    return p;
+}
+
 // n time steps, one launch (+ the stage-2 launch on sampled steps) each
 static int step_direct(lbm_s *h, int n)
 {
     for (int k = 0; k < n; ++k) {
         const bool sample = h->stats_every > 0 && (h->stats_phase % h->stats_every) == 0;
-        KParams p = h->kp;
-        if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
-        p.z0 = h->zlo; p.z1 = h->zhi;
-        if (sample) {
-            p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
-            p.shift = (h->mask || h->halo) ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
-        }
-        const bool timed = h->timing && h->ev_used + 2 <= 2 * MAX_TIMED;
-        if (timed) {
-            while (h->ev.size() < h->ev_used + 2) {
-                cudaEvent_t e;
-                CU_TRY(cudaEventCreate(&e));
-                h->ev.push_back(e);
-            }
-            CU_TRY(cudaEventRecord(h->ev[h->ev_used], h->stream));
-        }
-        CU_TRY(launch_step(h, p, sample));
-        if (timed) {
-            CU_TRY(cudaEventRecord(h->ev[h->ev_used + 1], h->stream));
-            h->ev_used += 2;
-        }
+        const KParams p = step_params(h, sample);
+        int rc = launch_step_timed(h, p, sample);
+        if (rc) return rc;
         if (sample) {
             CU_TRY(launch_stage2(h, 0));
             h->nsamples++;
@@ -1035,6 +1052,72 @@ int lbm_halo_pack(lbm_t *h, int side, float *buf_dev) { return halo_copy(h, side
 int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev)
 {
     return halo_copy(h, side, const_cast<float *>(buf_dev), false);
+}
+
+// One time step of a z slab, split so that the halo exchange overlaps the interior update:
+//   begin: update the two boundary planes, pack the faces of the NEW state, record `packed`,
+//          then launch the update of the interior planes;
+//   (caller: on another stream, wait for `packed`, exchange the buffers with the ring
+//    neighbours, record `ready`)
+//   end:   wait for `ready`, unpack into the ghost planes of the new state, statistics stage 2.
+int lbm_step_slab_begin(lbm_t *h, float *send_lo_dev, float *send_hi_dev, void *packed_event)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->halo) return fail(LBM_EINVAL, "handle was not created with LBM_Z_HALO");
+    if (!h->inited) return fail(LBM_ESTATE, "lbm_step_slab_begin before lbm_init / lbm_set_macros");
+    if (h->slab_open) return fail(LBM_ESTATE, "lbm_step_slab_begin twice without lbm_step_slab_end");
+    if (!send_lo_dev || !send_hi_dev) return fail(LBM_EINVAL, "send buffer is NULL");
+    const bool sample = h->stats_every > 0 && (h->stats_phase % h->stats_every) == 0;
+    KParams p = step_params(h, sample);
+    const int zl = h->zlo, zh = h->zhi;                   // interior planes [1, nz-1)
+    int rc;
+    p.z0 = zl; p.z1 = zl + 1;
+    if ((rc = launch_step_timed(h, p, sample))) return rc;
+    if (zh - 1 > zl) {
+        p.z0 = zh - 1; p.z1 = zh;
+        if ((rc = launch_step_timed(h, p, sample))) return rc;
+    }
+    const long long plane = (long long)h->nx * h->ny;
+    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
+    halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, 1, 0, send_lo_dev);
+    halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, h->nz - 2, 1, send_hi_dev);
+    h->launches += 2;
+    CU_TRY(cudaGetLastError());
+    if (packed_event) CU_TRY(cudaEventRecord(static_cast<cudaEvent_t>(packed_event), h->stream));
+    if (zh - 1 > zl + 1) {
+        p.z0 = zl + 1; p.z1 = zh - 1;
+        if ((rc = launch_step_timed(h, p, sample))) return rc;
+    }
+    h->slab_open = true; h->slab_sample = sample;
+    return LBM_OK;
+}
+
+int lbm_step_slab_end(lbm_t *h, const float *recv_lo_dev, const float *recv_hi_dev, void *ready_event)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->halo) return fail(LBM_EINVAL, "handle was not created with LBM_Z_HALO");
+    if (!h->slab_open) return fail(LBM_ESTATE, "lbm_step_slab_end without lbm_step_slab_begin");
+    if (!recv_lo_dev || !recv_hi_dev) return fail(LBM_EINVAL, "receive buffer is NULL");
+    if (ready_event) CU_TRY(cudaStreamWaitEvent(h->stream, static_cast<cudaEvent_t>(ready_event), 0));
+    const KParams p = step_params(h, false);              // p.dst holds state t+1
+    const long long plane = (long long)h->nx * h->ny;
+    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
+    // through the low face (ghost plane 0) come the c_z = +1 populations, through the high face
+    // (ghost plane nz-1) the c_z = -1 ones
+    halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, 0, 1, const_cast<float *>(recv_lo_dev));
+    halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, h->nz - 1, 0, const_cast<float *>(recv_hi_dev));
+    h->launches += 2;
+    CU_TRY(cudaGetLastError());
+    if (h->slab_sample) {
+        CU_TRY(launch_stage2(h, 0));
+        h->nsamples++;
+    }
+    if (h->stats_every > 0) h->stats_phase++;
+    h->t++;
+    h->slab_open = false;
+    return LBM_OK;
 }
 
 int lbm_stats_read_raw(lbm_t *h, double *out, double *centre, double *count)

@@ -1,10 +1,15 @@
 """z-slab decomposition of one lattice over several GPUs.
 
 Plumbing only: every population that moves is packed, unpacked and updated by the CUDA library
-(lbm_halo_pack / lbm_halo_unpack / lbm_step); this module decides WHO talks to WHOM and hands the
+(lbm_step_slab_begin / lbm_step_slab_end); this module decides WHO talks to WHOM and hands the
 packed device buffers to torch.distributed (NCCL point-to-point over NVLink) - one exchange of
 2 x 5 x nx x ny fp32 per time step ("only information from directly adjacent points is
 required") - and sums the [ny][10] raw statistics over the ranks at read-out.
+
+A step is split so that the exchange hides behind the interior update: the library updates the
+two boundary planes first, packs the faces and records an event; the exchange runs on a second
+CUDA stream that waits for that event while the library's stream updates the interior planes;
+the unpack waits for the exchange (lbm.h: lbm_step_slab_begin / _end).
 
 Rank r of W owns the global planes [r nz/W, (r+1) nz/W) plus one ghost plane on either side; z is
 periodic, so the ranks form a ring.  The slab uses the two-lattice storage (the in-place AA
@@ -67,6 +72,12 @@ class SlabLbm:
         self.cfg = cfg
         self._send = [self.sim.halo_buffer(), self.sim.halo_buffer()]    # [lo, hi]
         self._recv = [self.sim.halo_buffer(), self.sim.halo_buffer()]    # [from lower, from upper]
+        import torch
+
+        with torch.cuda.device(self.sim.device):
+            self._comm = torch.cuda.Stream(self.sim.device)              # the exchange runs here
+            self._packed = torch.cuda.Event()
+            self._ready = torch.cuda.Event()
 
     # -- halo exchange -----------------------------------------------------------------------
     def pack(self):
@@ -101,12 +112,25 @@ class SlabLbm:
     def stats_reset(self):
         self.sim.stats_reset()
 
-    def step(self, n: int = 1):
+    def step(self, n: int = 1, overlap: bool = True):
+        """n time steps.  overlap=True: boundary planes -> pack -> [exchange on the comm stream ||
+        interior planes] -> unpack; overlap=False: the sequential form (same bits)."""
         if self.emulated:
             raise RuntimeError("emulated slabs are advanced together: step_emulated(slabs, n)")
+        import torch
+
         for _ in range(int(n)):
-            self.sim.step(1)
-            self.exchange()
+            if not overlap:
+                self.sim.step(1)
+                self.exchange()
+                continue
+            self.sim.step_slab_begin(self._send[0], self._send[1], self._packed)
+            with torch.cuda.stream(self._comm):
+                self._comm.wait_event(self._packed)
+                ring_exchange(self._send[1], self._send[0], self._recv[0], self._recv[1], self.rank,
+                              self.world, self.group)
+                self._ready.record(self._comm)
+            self.sim.step_slab_end(self._recv[0], self._recv[1], self._ready)
 
     def get_macros(self):
         """(rho, u) of the interior planes: shapes (nz_local, ny, nx), (3, nz_local, ny, nx)."""
@@ -137,14 +161,36 @@ class SlabLbm:
         self.sim.close()
 
 
-def step_emulated(slabs, n: int = 1):
+def step_emulated(slabs, n: int = 1, overlap: bool = False):
     """Advance a list of slabs that live in ONE process (all ranks of a ring, e.g. on one GPU, one
-    after another - no kernel waits on another): same calls, the exchange done by local copies."""
+    after another - no kernel waits on another): same calls, the exchange done by local copies.
+    overlap=True drives the begin / exchange-on-a-second-stream / end form of SlabLbm.step."""
+    import torch
+
     W = len(slabs)
     for _ in range(int(n)):
+        if not overlap:
+            for s in slabs:
+                s.sim.step(1)
+            exchange_emulated(slabs)
+            continue
         for s in slabs:
-            s.sim.step(1)
-        exchange_emulated(slabs)
+            s.sim.step_slab_begin(s._send[0], s._send[1], s._packed)
+        for r, s in enumerate(slabs):
+            lower, upper = ring_neighbours(r, W)
+            with torch.cuda.stream(s._comm):
+                s._comm.wait_event(slabs[lower]._packed)
+                s._comm.wait_event(slabs[upper]._packed)
+                s._recv[0].copy_(slabs[lower]._send[1], non_blocking=True)
+                s._recv[1].copy_(slabs[upper]._send[0], non_blocking=True)
+                s._ready.record(s._comm)
+        for s in slabs:
+            s.sim.step_slab_end(s._recv[0], s._recv[1], s._ready)
+        # the next begin overwrites the send buffers: it must not overtake this step's copies
+        for s in slabs:
+            lower, upper = ring_neighbours(slabs.index(s), W)
+            torch.cuda.current_stream(s.sim.device).wait_event(slabs[lower]._ready)
+            torch.cuda.current_stream(s.sim.device).wait_event(slabs[upper]._ready)
 
 
 def init_emulated(slabs, seed: int):

@@ -159,3 +159,81 @@ def test_halo_flag_rules():
     g = lb.Lbm(32, 4, 6, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip"))
     with pytest.raises(lb.LbmError):
         g.set_z_slab(0, 4)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
+    """The begin / exchange-on-a-second-stream / end form (lbm_step_slab_begin/_end): re-assembled
+    slab fields against the ORACLE over 20 steps at the north_star tolerance, and bit for bit
+    against the undivided CUDA lattice (same arithmetic per cell)."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    cfg = wl.small(nx=64, ny=10, nz=12)
+    m = np.zeros((12, 10, 64), bool)
+    m[3:5, 0:3, 10:14] = True                            # a trip box across the face between slabs
+    cfg["solid"] = m
+    o = orc.Oracle.from_config(cfg)
+    o.init_from_config(cfg)
+    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref.init(cfg["seed"])
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True) for r in range(world)]
+    slab.init_emulated(slabs, cfg["seed"])
+    for s in slabs:
+        s.stats_accumulate(1)
+    o.stats_accumulate(1)
+    tol = 1e-5 * cfg["u_bulk"]
+    for n in (1, 2, 7, 10):
+        o.step(n)
+        ref.step(n)
+        slab.step_emulated(slabs, n, overlap=True)
+        torch.cuda.synchronize()
+        rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
+        us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
+        rr, ur = ref.get_macros()
+        assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
+        ro, uo = o.get_macros()
+        assert np.abs(rs.cpu().numpy() - ro).max() <= tol and np.abs(us.cpu().numpy() - uo).max() <= tol
+    so, no = o.stats_read()
+    ss = slab.stats_emulated(slabs)
+    assert no == 20
+    assert np.abs(ss[:, 0:3] - so[:, 0:3]).max() <= tol
+    assert np.abs(ss[:, 3:9] - so[:, 3:9]).max() <= tol * cfg["u_bulk"]
+    assert np.abs(ss[:, 9] - so[:, 9]).max() <= 1e-6
+    # begin twice / end without begin are refused
+    with pytest.raises(lb.LbmError):
+        slabs[0].sim.step_slab_end(slabs[0]._recv[0], slabs[0]._recv[1])
+    slabs[0].sim.step_slab_begin(slabs[0]._send[0], slabs[0]._send[1])
+    with pytest.raises(lb.LbmError):
+        slabs[0].sim.step_slab_begin(slabs[0]._send[0], slabs[0]._send[1])
+    for s in slabs:
+        s.close()
+
+
+@pytest.mark.gpu
+def test_single_slab_overlapped_through_the_comm_stream():
+    """world == 1 through SlabLbm.step(overlap=True): the exchange (self-periodic copies) runs on
+    the second stream between begin and end."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    cfg = wl.small(nx=64, ny=8, nz=6)
+    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref.init(3)
+    a = slab.SlabLbm(cfg, 0, 1)
+    b = slab.SlabLbm(cfg, 0, 1)
+    a.init(3)
+    b.init(3)
+    ref.step(9)
+    a.step(9, overlap=True)
+    b.step(9, overlap=False)
+    torch.cuda.synchronize()
+    assert torch.equal(a.get_macros()[1], ref.get_macros()[1])
+    assert torch.equal(b.get_macros()[1], ref.get_macros()[1])
