@@ -78,6 +78,10 @@ class SlabLbm:
             self._comm = torch.cuda.Stream(self.sim.device)              # the exchange runs here
             self._packed = torch.cuda.Event()
             self._ready = torch.cuda.Event()
+            # torch creates the CUDA event at the first record(): make the handles real now, they
+            # are handed to the library as raw cudaEvent_t
+            self._packed.record()
+            self._ready.record()
 
     # -- halo exchange -----------------------------------------------------------------------
     def pack(self):

@@ -112,7 +112,14 @@ def test_emulated_slabs_equal_global_lattice(world, case):
         rr, ur = ref.get_macros()
         rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
         us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
-        assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
+        if case == "forest":
+            assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
+        else:
+            # geometry handles run the plain or the geometry body per thread block (two
+            # instantiations of the same arithmetic: ptxas contracts their FMAs differently when the
+            # statistics are fused in), so a different block decomposition may round a cell
+            # differently: equal to a few ulp, not bit for bit
+            assert float((rs - rr).abs().max()) <= 2e-7 and float((us - ur).abs().max()) <= 5e-8, (world, n)
     sr, nr = ref.stats_read()
     ss = slab.stats_emulated(slabs)
     assert nr == 9
@@ -165,8 +172,9 @@ def test_halo_flag_rules():
 @pytest.mark.parametrize("world", [1, 2, 3])
 def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
     """The begin / exchange-on-a-second-stream / end form (lbm_step_slab_begin/_end): re-assembled
-    slab fields against the ORACLE over 20 steps at the north_star tolerance, and bit for bit
-    against the undivided CUDA lattice (same arithmetic per cell)."""
+    slab fields against the ORACLE over 20 steps at the north_star tolerance, and to a few ulp
+    against the undivided CUDA lattice (a geometry handle: see the note in the test above; without
+    geometry the slabs are bit-identical, test_single_slab_overlapped_through_the_comm_stream)."""
     import torch
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
@@ -195,7 +203,7 @@ def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
         rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
         us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
         rr, ur = ref.get_macros()
-        assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
+        assert float((rs - rr).abs().max()) <= 2e-7 and float((us - ur).abs().max()) <= 5e-8, (world, n)
         ro, uo = o.get_macros()
         assert np.abs(rs.cpu().numpy() - ro).max() <= tol and np.abs(us.cpu().numpy() - uo).max() <= tol
     so, no = o.stats_read()
