@@ -516,6 +516,9 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes (read+write) per step-kernel launch, from profiles/, to quote in the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--boxes", action="store_true",
+                    help="geometry handle with the paper's turbulence-trip boxes in place (PAPER.md:L226): "
+                         "times the geometry variants of the kernels")
     ap.add_argument("--sharded", action="store_true",
                     help="one lattice cut into N z slabs with a halo exchange per step (opt-in)")
     args = ap.parse_args()
@@ -531,6 +534,10 @@ def main():
         cfg["storage"] = args.storage
     if args.stats_every is not None:
         cfg["stats_every"] = args.stats_every
+    if args.boxes:
+        from paper_2206_15454_b200.run_paper_cases import trip_boxes
+        cfg["solid"] = trip_boxes(cfg)
+        cfg["note"] += ", trip boxes in place (geometry kernels)"
     if args.impl == "reference":
         return run_reference(args, cfg)
     if args.sharded:
