@@ -42,7 +42,8 @@ BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star; DESIGN.md "Roo
 # of the current kernels on the named config (profiles/): the line quotes the figure of its own
 # config when one exists, else null.
 NCU_TRAFFIC_BYTES_PER_CELL = {
-    ("cfg4", "aa"): (151.7, "profiles/r01_README.md, ncu --set full on cfg4, both AA parities"),
+    ("cfg5", "aa"): (152.1, "profiles/r02_README.md, ncu dram__bytes_read+write on cfg5 itself, both AA parities"),
+    ("cfg4", "aa"): (151.7, "profiles/r02_README.md, ncu --set full on cfg4, both AA parities"),
     ("cfg3", "two_lattice"): (149.0, "profiles/r01_README.md, ncu --set full on cfg3"),
 }
 METRIC = "MLUPS"
@@ -199,7 +200,7 @@ def run_reference(args, cfg):
 
 
 def workload_config(cfg, args, variant):
-    pops_gb = wl.n_cells(cfg) * 76 * (1 if cfg["storage"] == "aa" else 2) / 1e9
+    pops_gb = wl.n_cells(cfg) * 76 * (1 if cfg["storage"] in ("aa", "aax") else 2) / 1e9
     c = {
         "workload": f"{cfg['name']}: {cfg['note']}",
         "lattice": [cfg["nx"], cfg["ny"], cfg["nz"]], "cells": wl.n_cells(cfg),
@@ -260,9 +261,8 @@ def run_b200(args, cfg):
 
     K, W = args.steps, args.warmup
     N = wl.n_cells(cfg)
-    aa = cfg["storage"] == "aa"
     every = cfg.get("stats_every", 0)
-    sim = lb.Lbm.from_config(cfg, aa=aa, device=dev)
+    sim = lb.Lbm.from_config(cfg, device=dev)          # storage scheme from cfg["storage"]
     if args.shape:
         tx, ty = (int(v) for v in args.shape.split("x"))
         sim.set_launch_shape(tx, ty)
@@ -507,7 +507,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 (BASELINE.json:configs[0..4])")
-    ap.add_argument("--storage", choices=["aa", "two_lattice"], default=None,
+    ap.add_argument("--storage", choices=["aa", "aax", "two_lattice"], default=None,
                     help="override the config's storage scheme")
     ap.add_argument("--stats-every", type=int, default=None, help="override the config's stats cadence")
     ap.add_argument("--shape", default=None, help="thread-block shape override TXxTY (tuning)")

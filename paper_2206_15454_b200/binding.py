@@ -21,6 +21,7 @@ SOLID_MASK = 1 << 5
 STORAGE_AA = 1 << 6
 Z_HALO = 1 << 7
 VEC_SHIFT = 8
+STORAGE_AAX = 1 << 11
 NSTAT = 10
 
 INIT_POWER_LAW, INIT_PARABOLA, INIT_REST = 0, 1, 2
@@ -125,9 +126,11 @@ def _check(rc: int):
         raise LbmError(rc, lib().lbm_last_error().decode())
 
 
-def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa: bool = False, vec: int = 0,
+def bc_flags(bottom: str, top: str, drag_vector: bool = False, aa=False, vec: int = 0,
              solid: bool = False, halo: bool = False) -> int:
-    return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0) | (STORAGE_AA if aa else 0)
+    """aa: False = two-lattice, True / "aa" = AA pattern, "aax" = x-balanced AA pattern."""
+    storage = STORAGE_AAX if aa == "aax" else (STORAGE_AA if aa else 0)
+    return (_BOTTOM[bottom] | _TOP[top] | (DRAG_VECTOR if drag_vector else 0) | storage
             | (SOLID_MASK if solid else 0) | (Z_HALO if halo else 0) | (int(vec) << VEC_SHIFT))
 
 
@@ -263,7 +266,8 @@ class Lbm:
     @classmethod
     def from_config(cls, cfg: dict, aa=None, vec: int = 0, halo: bool = False, **kw) -> "Lbm":
         if aa is None:
-            aa = cfg.get("storage", "two_lattice") == "aa"
+            st = cfg.get("storage", "two_lattice")
+            aa = "aax" if st == "aax" else (st == "aa")
         flags = bc_flags(cfg["bottom"], cfg["top"], cfg.get("drag_vector", False), aa, vec,
                          solid=cfg.get("solid") is not None or cfg.get("forest_cells") is not None
                          or cfg.get("geometry", False), halo=halo)

@@ -13,14 +13,19 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 SRC = [os.path.join(_HERE, "csrc", "lbm_api.cu")]
-DEPS = SRC + [os.path.join(_HERE, "csrc", "lbm_kernels.cuh"), os.path.join(ROOT, "include", "lbm.h")]
+DEPS = SRC + [os.path.join(_HERE, "csrc", "lbm_kernels.cuh"), os.path.join(_HERE, "csrc", "lbm_tma.cuh"),
+              os.path.join(ROOT, "include", "lbm.h")]
 LIB = os.path.join(_HERE, "liblbm_b200.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared",
-    "--fmad=true",            # FMA contraction on; no -use_fast_math (IEEE sqrt / division)
+    # FMA contraction on.  No -use_fast_math: the kernels choose their approximations themselves -
+    # MUFU rcp.approx / sqrt.approx with FTZ (inline PTX in lbm_kernels.cuh) for 1/rho, |u|, the two
+    # square roots of Eqs. 11-12 and 1/tau, where the error is second order (DESIGN.md "Arithmetic
+    # form"); everything else is IEEE fp32.
+    "--fmad=true",
     "-Xptxas", "-warn-spills", "-diag-suppress", "177",
 ]
 

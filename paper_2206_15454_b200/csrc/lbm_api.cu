@@ -92,7 +92,7 @@ struct lbm_s {
     std::vector<double> lad;
     uint32_t bc;
     int bot, top;
-    bool aa, drag_vector, mask, halo;
+    bool aa, aax, drag_vector, mask, halo;   // aax: the x-balanced variant of the AA pattern (aa is set too)
     bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
     bool forest_codes;          // per-cell forest codes installed (geometry handles)
     bool slab_open, slab_sample; // between lbm_step_slab_begin and _end; that step samples
@@ -157,7 +157,8 @@ static void set_variant(lbm_s *h)
 {
     char tma[32] = "";
     if (h->tma_mode) snprintf(tma, sizeof(tma), "/tma%dx%d", h->tma_mode, h->tma_rows);
-    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d%s", h->aa ? "aa" : "pull2", h->V, h->TX, h->TY, tma);
+    snprintf(h->variant, sizeof(h->variant), "%s/v%d/tx%dx%d%s", h->aax ? "aax" : (h->aa ? "aa" : "pull2"), h->V,
+             h->TX, h->TY, tma);
 }
 
 // The statistics partials are laid out with `pchunks` x chunks per row: the larger of the
@@ -225,7 +226,8 @@ int lbm_workspace_bytes(int nx, int ny, int nz, uint32_t bc_flags, size_t *bytes
     if (!bytes) return fail(LBM_EINVAL, "bytes is NULL");
     if (nx < 1 || ny < 1 || nz < 1) return fail(LBM_EINVAL, "lattice sizes must be >= 1");
     if ((double)nx * ny * nz >= 2147483648.0) return fail(LBM_EINVAL, "nx*ny*nz must be < 2^31");
-    *bytes = make_layout(nx, ny, nz, (bc_flags & LBM_STORAGE_AA) != 0, (bc_flags & LBM_SOLID_MASK) != 0).total;
+    *bytes = make_layout(nx, ny, nz, (bc_flags & (LBM_STORAGE_AA | LBM_STORAGE_AAX)) != 0,
+                         (bc_flags & LBM_SOLID_MASK) != 0).total;
     return LBM_OK;
 }
 
@@ -239,12 +241,14 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     if (!(nu > 0.0) || !std::isfinite(nu)) return fail(LBM_EINVAL, "nu must be > 0 (got %g)", nu);
     if (!(Cs >= 0.0) || !std::isfinite(Cs)) return fail(LBM_EINVAL, "Cs must be >= 0 (got %g)", Cs);
     if (!(Cd >= 0.0) || !std::isfinite(Cd)) return fail(LBM_EINVAL, "Cd must be >= 0 (got %g)", Cd);
-    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_SOLID_MASK | LBM_STORAGE_AA | LBM_Z_HALO | LBM_VEC_MASK))
+    if (bc_flags & ~(0xFu | LBM_DRAG_VECTOR | LBM_SOLID_MASK | LBM_STORAGE_AA | LBM_STORAGE_AAX | LBM_Z_HALO | LBM_VEC_MASK))
         return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
     int bot, top;
     if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
+    if ((bc_flags & LBM_STORAGE_AAX) && (bc_flags & LBM_SOLID_MASK))
+        return fail(LBM_EINVAL, "LBM_STORAGE_AAX has no geometry variant: use LBM_STORAGE_AA or two-lattice storage with LBM_SOLID_MASK");
     if (bc_flags & LBM_Z_HALO) {
-        if (bc_flags & LBM_STORAGE_AA) return fail(LBM_EINVAL, "LBM_Z_HALO needs two-lattice storage");
+        if (bc_flags & (LBM_STORAGE_AA | LBM_STORAGE_AAX)) return fail(LBM_EINVAL, "LBM_Z_HALO needs two-lattice storage");
         if (nz < 3) return fail(LBM_EINVAL, "LBM_Z_HALO needs nz >= 3 (two ghost planes + >= 1 interior)");
     }
     const int V = pick_vec(nx, bc_flags);
@@ -264,7 +268,8 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
             h->lad[j] = lad_profile[j];
         }
     h->bc = bc_flags; h->bot = bot; h->top = top;
-    h->aa = (bc_flags & LBM_STORAGE_AA) != 0;
+    h->aax = (bc_flags & LBM_STORAGE_AAX) != 0;
+    h->aa = h->aax || (bc_flags & LBM_STORAGE_AA) != 0;    // both are single-array schemes
     h->drag_vector = (bc_flags & LBM_DRAG_VECTOR) != 0;
     h->V = V;
     h->mask = (bc_flags & LBM_SOLID_MASK) != 0;
@@ -279,7 +284,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
         return fail(LBM_EINVAL, "no block shape for nx=%d with %d cells per thread", nx, V);
     }
     h->nchunk = (nx / V) / h->TX;
-    h->tma_ok = (V == 4) && (nx % TMA_BOX == 0) && !h->mask;
+    h->tma_ok = (V == 4) && (nx % TMA_BOX == 0) && !h->mask && !h->aax;
     h->tma_rows = (ny % 2 == 0) ? 2 : 1;
     h->tma_mode = 0;
     if (h->tma_ok) {
@@ -636,7 +641,8 @@ static cudaError_t launch_init_v(lbm_s *h, const KParams &p, int planes)
     if (h->mask) {
         if (h->aa) init_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p);
         else init_kernel<V, WR_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
-    } else if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
+    } else if (h->aax) init_kernel<V, WR_XO><<<grid, block, 0, h->stream>>>(p);
+    else if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
     else init_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
     return cudaGetLastError();
@@ -659,6 +665,8 @@ static cudaError_t launch_macros_v(lbm_s *h, const KParams &p, int planes)
         else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
         else macros_kernel<V, RD_PULL_OPP, true><<<grid, block, 0, h->stream>>>(p);
     } else if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
+    else if (h->aax && (h->t & 1) == 0) macros_kernel<V, RD_XE><<<grid, block, 0, h->stream>>>(p);
+    else if (h->aax) macros_kernel<V, RD_XO><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL><<<grid, block, 0, h->stream>>>(p);
     else macros_kernel<V, RD_PULL_OPP><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
@@ -717,6 +725,8 @@ static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
         else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S, true><<<grid, block, 0, h->stream>>>(p);
         else step_kernel<V, RD_PULL_OPP, WR_PUSH, S, true><<<grid, block, 0, h->stream>>>(p);
     } else if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
+    else if (h->aax && (h->t & 1) == 0) step_kernel<V, RD_XE, WR_XE, S><<<grid, block, 0, h->stream>>>(p);
+    else if (h->aax) step_kernel<V, RD_XO, WR_XO, S><<<grid, block, 0, h->stream>>>(p);
     else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S><<<grid, block, 0, h->stream>>>(p);
     else step_kernel<V, RD_PULL_OPP, WR_PUSH, S><<<grid, block, 0, h->stream>>>(p);
     h->launches++;
@@ -1255,6 +1265,8 @@ int lbm_get_state(lbm_t *h, float *out_dev)
     KParams p = read_params(h);
     const unsigned blocks = (unsigned)((h->N + 255) / 256);
     if (!h->aa) state_kernel<0><<<blocks, 256, 0, h->stream>>>(p, out_dev);
+    else if (h->aax && (h->t & 1)) state_kernel<3><<<blocks, 256, 0, h->stream>>>(p, out_dev);
+    else if (h->aax) state_kernel<4><<<blocks, 256, 0, h->stream>>>(p, out_dev);
     else if (h->t & 1) state_kernel<1><<<blocks, 256, 0, h->stream>>>(p, out_dev);
     else state_kernel<2><<<blocks, 256, 0, h->stream>>>(p, out_dev);
     h->launches++;
@@ -1271,6 +1283,8 @@ static cudaError_t launch_setstate_v(lbm_s *h, const KParams &p, const float *in
         else if (odd) setstate_kernel<V, WR_LOCAL_OPP, true><<<grid, block, 0, h->stream>>>(p, in);
         else setstate_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p, in);
     } else if (!h->aa) setstate_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p, in);
+    else if (h->aax && odd) setstate_kernel<V, WR_XE><<<grid, block, 0, h->stream>>>(p, in);
+    else if (h->aax) setstate_kernel<V, WR_XO><<<grid, block, 0, h->stream>>>(p, in);
     else if (odd) setstate_kernel<V, WR_LOCAL_OPP><<<grid, block, 0, h->stream>>>(p, in);
     else setstate_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p, in);
     h->launches++;

@@ -43,14 +43,29 @@ struct Lat {
 
 // How the streamed (pre-collision) populations of a cell are fetched / how the post-collision
 // ones are put back.
-enum ReadMode { RD_LOCAL = 0,   // A[i][x]                         (AA even step; AA state, t even)
-                RD_PULL = 1,    // A[i][x - c_i]                   (two-lattice)
-                RD_PULL_OPP = 2 // A[opp i][x - c_i]               (AA odd step; AA state, t odd)
+enum ReadMode { RD_LOCAL = 0,    // A[i][x]                         (AA even step; AA state, t even)
+                RD_PULL = 1,     // A[i][x - c_i]                   (two-lattice)
+                RD_PULL_OPP = 2, // A[opp i][x - c_i]               (AA odd step; AA state, t odd)
+                RD_XE = 3,       // x-balanced AA, even step        (see below)
+                RD_XO = 4        // x-balanced AA, odd step
 };
 enum WriteMode { WR_LOCAL = 0,     // B[i][x]                      (two-lattice)
                  WR_LOCAL_OPP = 1, // A[opp i][x]                  (AA even step)
-                 WR_PUSH = 2       // A[i][x + c_i]                (AA odd step, AA init)
+                 WR_PUSH = 2,      // A[i][x + c_i]                (AA odd step, AA init)
+                 WR_XE = 3,        // x-balanced AA, even step
+                 WR_XO = 4         // x-balanced AA, odd step
 };
+// x-balanced AA ("AAX").  In the AA pattern the even step touches only its own cell and the odd
+// step does all the streaming: 10 x-shifted reads and 10 x-shifted writes, which on 128-bit
+// accesses cost shuffles and scalar edge accesses, so the odd step is issue-bound where the even
+// one is bandwidth-bound.  Any in-place scheme is hazard-free as long as every cell writes exactly
+// the locations it read; that leaves the freedom to keep the x part of the displacement of some
+// populations for the other step.  With a_i = 1 for c_ix = +1 (else 0), population i of cell x
+// lives at slot i, cell x + c_i - a_i e_x after an odd step and at slot opp(i), cell x - a_opp(i) e_x
+// after an even step.  Net effect, identical in BOTH steps and independent of wall / free-slip
+// redirections (which only change slot and row, as in AA): populations with c_x = +1 are READ from
+// x - 1, populations with c_x = -1 are WRITTEN to x - 1, nothing else moves in x.  Each step then
+// has 5 x-shifted reads and 5 x-shifted writes; rows (y, z) and slots follow AA exactly.
 
 enum { BC_BOT_WALL = 0, BC_BOT_PERIODIC = 1 };
 enum { BC_TOP_WALL = 0, BC_TOP_SLIP = 1, BC_TOP_PERIODIC = 2, BC_TOP_LID = 3 };
@@ -182,44 +197,53 @@ __device__ __forceinline__ void load_dir(const KParams &p, const Ctx &c, float (
         ldv<V>(p.src + (long long)I * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), o);
         return;
     } else {
-        constexpr int S_N = (RM == RD_PULL) ? I : Lat::opp[I];
-        constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[I] : I;
-        constexpr int S_FS = (RM == RD_PULL) ? Lat::mir[I] : Lat::opp[Lat::mir[I]];
+        constexpr bool AAX = (RM == RD_XE || RM == RD_XO);
+        // the fetch comes from x - XS; the classic modes cancel the shift on a bounce-back link
+        constexpr int XS = AAX ? (cx == 1 ? 1 : 0) : cx;
         bool bb = false, fs = false;
-        if constexpr (cy == 1) bb = c.bot_bb;
-        if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
-        const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.ym : c.yp);
-        const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zm : c.zp);
-        const int slot = bb ? S_BB : (fs ? S_FS : S_N);
-        const int yrow = (bb || fs) ? c.y : ysel;
-        const int zrow = bb ? c.z : zsel;
-        const float *rowp = p.src + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
-        if constexpr (cx == 0) {
+        const float *rowp;
+        if constexpr (RM == RD_XE) {
+            rowp = p.src + (long long)I * p.N + (long long)(c.y + p.ny * c.z) * p.nx;
+        } else {
+            constexpr int S_N = (RM == RD_PULL) ? I : Lat::opp[I];
+            constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[I] : I;
+            constexpr int S_FS = (RM == RD_PULL) ? Lat::mir[I] : Lat::opp[Lat::mir[I]];
+            if constexpr (cy == 1) bb = c.bot_bb;
+            if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
+            const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.ym : c.yp);
+            const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zm : c.zp);
+            const int slot = bb ? S_BB : (fs ? S_FS : S_N);
+            const int yrow = (bb || fs) ? c.y : ysel;
+            const int zrow = bb ? c.z : zsel;
+            rowp = p.src + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
+        }
+        const bool cancel = AAX ? false : bb;
+        if constexpr (XS == 0) {
             ldv<V>(rowp + c.x0, o);
         } else if constexpr (V == 1) {
-            const int xs = bb ? c.x0 : (cx == 1 ? c.xl : c.xr);
+            const int xs = cancel ? c.x0 : (XS == 1 ? c.xl : c.xr);
             o[0] = rowp[xs];
         } else {
             float v[V];
             ldv<V>(rowp + c.x0, v);
-            if constexpr (cx == 1) {           // need x0-1 .. x0+V-2
-                const bool need = c.edgeL && !bb;
+            if constexpr (XS == 1) {           // need x0-1 .. x0+V-2
+                const bool need = c.edgeL && !cancel;
                 float e = 0.f;
                 if (need) e = rowp[c.xl];
                 float l = __shfl_up_sync(0xffffffffu, v[V - 1], 1);
                 l = c.edgeL ? e : l;
-                o[0] = bb ? v[0] : l;
+                o[0] = cancel ? v[0] : l;
 #pragma unroll
-                for (int k = 1; k < V; ++k) o[k] = bb ? v[k] : v[k - 1];
+                for (int k = 1; k < V; ++k) o[k] = cancel ? v[k] : v[k - 1];
             } else {                            // need x0+1 .. x0+V
-                const bool need = c.edgeR && !bb;
+                const bool need = c.edgeR && !cancel;
                 float e = 0.f;
                 if (need) e = rowp[c.xr];
                 float r = __shfl_down_sync(0xffffffffu, v[0], 1);
                 r = c.edgeR ? e : r;
 #pragma unroll
-                for (int k = 0; k < V - 1; ++k) o[k] = bb ? v[k] : v[k + 1];
-                o[V - 1] = bb ? v[V - 1] : r;
+                for (int k = 0; k < V - 1; ++k) o[k] = cancel ? v[k] : v[k + 1];
+                o[V - 1] = cancel ? v[V - 1] : r;
             }
         }
     }
@@ -238,31 +262,40 @@ template <int V, int WM, int I>
 __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const float (&r)[V], bool act = true)
 {
     constexpr int cx = Lat::cx[I], cy = Lat::cy[I], cz = Lat::cz[I];
-    if constexpr (WM != WR_PUSH) {
+    if constexpr (WM == WR_LOCAL || WM == WR_LOCAL_OPP) {
         constexpr int S = (WM == WR_LOCAL) ? I : Lat::opp[I];
         stv<V>(p.dst + (long long)S * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), r);
         return;
     } else {
+        constexpr bool AAX = (WM == WR_XE || WM == WR_XO);
+        // the values land on x + XS; the classic push cancels the shift on a bounce-back link
+        constexpr int XS = AAX ? (cx == -1 ? -1 : 0) : cx;
         bool bb = false, fs = false;
-        if constexpr (cy == -1) bb = c.bot_bb;
-        if constexpr (cy == 1) { bb = c.top_bb; fs = c.top_fs; }
-        const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.yp : c.ym);
-        const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zp : c.zm);
-        constexpr int S_BB = Lat::opp[I], S_FS = Lat::mir[I];
-        const int slot = bb ? S_BB : (fs ? S_FS : I);
-        const int yrow = (bb || fs) ? c.y : ysel;
-        const int zrow = bb ? c.z : zsel;
-        float *rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
-        if constexpr (cx == 0) {
+        float *rowp;
+        if constexpr (WM == WR_XE) {
+            rowp = p.dst + (long long)Lat::opp[I] * p.N + (long long)(c.y + p.ny * c.z) * p.nx;
+        } else {
+            if constexpr (cy == -1) bb = c.bot_bb;
+            if constexpr (cy == 1) { bb = c.top_bb; fs = c.top_fs; }
+            const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.yp : c.ym);
+            const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zp : c.zm);
+            constexpr int S_BB = Lat::opp[I], S_FS = Lat::mir[I];
+            const int slot = bb ? S_BB : (fs ? S_FS : I);
+            const int yrow = (bb || fs) ? c.y : ysel;
+            const int zrow = bb ? c.z : zsel;
+            rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zrow) * p.nx;
+        }
+        const bool cancel = AAX ? false : bb;
+        if constexpr (XS == 0) {
             if (act) stv<V>(rowp + c.x0, r);
         } else if constexpr (V == 1) {
-            const int xs = bb ? c.x0 : (cx == 1 ? c.xr : c.xl);
+            const int xs = cancel ? c.x0 : (XS == 1 ? c.xr : c.xl);
             if (act) rowp[xs] = r[0];
         } else {
-            if constexpr (cx == 1) {           // values land on x0+1 .. x0+V
+            if constexpr (XS == 1) {           // values land on x0+1 .. x0+V
                 const float l = __shfl_up_sync(0xffffffffu, r[V - 1], 1);
                 if (!act) {
-                } else if (bb) {
+                } else if (cancel) {
                     stv<V>(rowp + c.x0, r);
                 } else {
                     if (!c.edgeL) {
@@ -280,7 +313,7 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
             } else {                            // values land on x0-1 .. x0+V-2
                 const float rr = __shfl_down_sync(0xffffffffu, r[0], 1);
                 if (!act) {
-                } else if (bb) {
+                } else if (cancel) {
                     stv<V>(rowp + c.x0, r);
                 } else {
                     if (!c.edgeR) {
@@ -416,6 +449,7 @@ __device__ __forceinline__ void solid_fix_loads(const KParams &p, const Ctx &c, 
                                                 unsigned long long S)
 {
     if constexpr (RM == RD_LOCAL) return;
+    static_assert(RM == RD_LOCAL || RM == RD_PULL || RM == RD_PULL_OPP, "the geometry variants exist for two-lattice and AA storage");
     static_for<1, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
@@ -445,6 +479,7 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float 
             store_dir<V, WM, i>(p, c, g[i]);
         });
     } else if constexpr (WM != WR_PUSH) {
+        static_assert(WM == WR_LOCAL || WM == WR_LOCAL_OPP, "the geometry variants exist for two-lattice and AA storage");
         const unsigned self = solid_self<V>(S);
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
@@ -828,7 +863,7 @@ __device__ __forceinline__ void step_body(const KParams &p)
         }
         collide<V>(p, g, k, m, jr);
     }
-    const Ctx c2 = (WM == WR_PUSH) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
+    const Ctx c2 = (WM == WR_PUSH || WM == WR_XO) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
     if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
     else store_all<V, WM, false>(p, c2, g);
     if constexpr (STATS) {
@@ -1088,6 +1123,8 @@ __global__ void mask_change_kernel(const KParams p, float *arr, const unsigned *
 //   AA, t odd            : src[opp i][x]
 //   AA, t even (PUSH)    : src[i][x + c_i] with the wall / free-slip / solid redirections of
 //                          store_all; solid cells report the rest state (0)
+//   AAX, t odd  (MODE 3) : src[opp i][x - 1 if c_x = -1 else x]
+//   AAX, t even (MODE 4) : as PUSH in slot, y and z; in x: x - 1 if c_x = -1 else x
 template <int MODE>
 __global__ void state_kernel(const KParams p, float *out)
 {
@@ -1102,21 +1139,27 @@ __global__ void state_kernel(const KParams p, float *out)
         constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
         constexpr int S_OPP = Lat::opp[i], S_MIR = Lat::mir[i];
         float v;
+        // x-balanced AA: in every representation only the c_x = -1 populations sit one cell to the left
+        constexpr int xdx = (cx == -1) ? -1 : 0;
         if constexpr (MODE == 0) v = p.src[(long long)i * p.N + cell];
         else if constexpr (MODE == 1) v = p.src[(long long)S_OPP * p.N + cell];
-        else {
-            int slot = i, xd = x + cx, yd = y + cy, zd = z + cz;
+        else if constexpr (MODE == 3) {
+            int xd = x + xdx;
+            xd = (xd < 0) ? p.nx - 1 : xd;
+            v = p.src[(long long)S_OPP * p.N + (cell - x + xd)];
+        } else {
+            int slot = i, xd = x + (MODE == 4 ? xdx : cx), yd = y + cy, zd = z + cz;
             xd = (xd < 0) ? p.nx - 1 : (xd >= p.nx ? 0 : xd);
             zd = (zd < 0) ? p.nz - 1 : (zd >= p.nz ? 0 : zd);
             if (yd < 0) {
                 if (p.bot == BC_BOT_PERIODIC) yd = p.ny - 1;
-                else { slot = S_OPP; xd = x; yd = y; zd = z; }
+                else { slot = S_OPP; xd = (MODE == 4) ? xd : x; yd = y; zd = z; }
             } else if (yd >= p.ny) {
                 if (p.top == BC_TOP_PERIODIC) yd = 0;
                 else if (p.top == BC_TOP_SLIP) { slot = S_MIR; yd = y; }
-                else { slot = S_OPP; xd = x; yd = y; zd = z; }
+                else { slot = S_OPP; xd = (MODE == 4) ? xd : x; yd = y; zd = z; }
             }
-            if (solid_at(p, xd, yd, zd)) { slot = S_OPP; xd = x; yd = y; zd = z; }
+            if (MODE == 2 && solid_at(p, xd, yd, zd)) { slot = S_OPP; xd = x; yd = y; zd = z; }
             v = p.src[(long long)slot * p.N + ((long long)(yd + p.ny * zd) * p.nx + xd)];
         }
         out[(long long)i * p.N + cell] = self_solid ? 0.f : v;

@@ -5,8 +5,11 @@ The CUDA path and the fp64 oracle start from the same seeded field, spin up, the
 y-plane statistics over the same window.  By then the two trajectories differ locally by far more
 than the 100-step tolerance (asserted, so that the test really is about diverged runs); what must
 still agree is the statistics.  Differences are normalised by the profile maxima, as north_star's
-percentages are read in DESIGN.md §4.  Lattices are the ones the oracle finishes in seconds; the
-full-length config-2 window (20 k + 20 k steps) is listed in DESIGN.md §10 as not run.
+percentages are read in DESIGN.md §4 ("of the profile maximum"), and additionally point by point
+relative to the local value wherever the profile exceeds a fifth of its maximum (near zero
+crossings a relative bound means nothing).  Lattices are the ones the oracle finishes in seconds:
+these are small-lattice, short-window checks; the full-length config-2 run (20 k + 20 k steps, one
+hour of oracle time) is tests/run_p11_cfg2.py, its report profiles/r01_p11_cfg2.md.
 """
 import numpy as np
 import pytest
@@ -69,11 +72,23 @@ def test_long_run_statistics(orc, gpu, case, aa, spin, window):
     if case == "cfg1":
         assert diverged > 10 * 1e-5 * cfg["u_bulk"]
     assert d_mean <= 0.02
+
+    def pointwise(k):
+        """worst |difference| / |oracle value| over the rows whose value exceeds 20 % of the maximum"""
+        rows = np.abs(so[:, k]) >= 0.2 * np.abs(so[:, k]).max()
+        rel = np.abs(sg[rows, k] - so[rows, k]) / np.abs(so[rows, k])
+        j = int(np.flatnonzero(rows)[int(np.argmax(rel))])
+        return float(rel.max()), j
+
+    rel, j = pointwise(0)
+    print(f"   <U>: worst pointwise relative difference {100 * rel:.3f} % at row {j}")
+    assert rel <= 0.02
     for k, name in ((3, "uu"), (4, "vv"), (5, "ww"), (6, "uv")):
         m = np.abs(so[:, k]).max()
         d = np.abs(sg[:, k] - so[:, k]).max() / m
-        print(f"   <{name}>: max {m:.3e}, differs by {100 * d:.3f} % of max")
-        assert d <= 0.05
+        rel, j = pointwise(k)
+        print(f"   <{name}>: max {m:.3e}, differs by {100 * d:.3f} % of max, pointwise {100 * rel:.3f} % at row {j}")
+        assert d <= 0.05 and rel <= 0.05
     # the near-zero stresses (vw, uw vanish by symmetry) are compared on the scale of uv
     scale = np.abs(so[:, 6]).max()
     assert np.abs(sg[:, 7:9] - so[:, 7:9]).max() <= 0.05 * scale

@@ -69,7 +69,7 @@ def _state_err(o, g, w):
 BCS = [(wl.BOUNCE_BACK, wl.FREE_SLIP), (wl.BOUNCE_BACK, wl.BOUNCE_BACK), (wl.PERIODIC, wl.PERIODIC)]
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("nx,vec", [(32, 4), (32, 2), (32, 1), (36, 4), (34, 2), (33, 1), (128, 4),
                                     (256, 4), (4, 4), (2, 2), (1, 1), (200, 4), (1536, 4)])
 @pytest.mark.parametrize("bottom,top", BCS, ids=["wall-slip", "wall-wall", "periodic"])
@@ -78,7 +78,7 @@ def test_small_state_and_macros(orc, gpu, aa, nx, vec, bottom, top):
     cfg = wl.small(nx=nx, ny=ny, nz=nz, bottom=bottom, top=top, drag_vector=False)
     o, g = _pair(orc, gpu, cfg, aa, vec)
     w = _weights(orc)
-    assert f"v{vec}" in g.variant and (("aa" in g.variant) == aa)
+    assert f"v{vec}" in g.variant and g.variant.startswith({False: "pull2/", True: "aa/", "aax": "aax/"}[aa])
     assert _state_err(o, g, w) <= 2e-8            # state 0
     er, eu = _macro_err(o, g)
     assert er <= 2e-7 and eu <= 2e-8
@@ -91,7 +91,7 @@ def test_small_state_and_macros(orc, gpu, aa, nx, vec, bottom, top):
         assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 def test_vector_drag_and_general_force(orc, gpu, aa):
     cfg = wl.small(nx=64, ny=10, nz=8, drag_vector=True)
     cfg["body_force"] = (2e-6, -1e-6, 5e-7)
@@ -111,7 +111,7 @@ def test_degenerate_lattices(orc, gpu, shape, bottom, top):
     nx, ny, nz = shape
     cfg = wl.small(nx=nx, ny=ny, nz=nz, bottom=bottom, top=top, forest_rows=min(1, ny))
     w = _weights(orc)
-    for aa in (False, True):
+    for aa in (False, True, "aax"):
         o, g = _pair(orc, gpu, cfg, aa, 0)
         assert _state_err(o, g, w) <= 5e-8
         for n in (1, 2, 0, 5):
@@ -132,7 +132,7 @@ def test_single_block_shapes(orc, gpu):
     o.stats_accumulate(1)
     o.step(4)
     so, _ = o.stats_read()
-    for aa in (False, True):
+    for aa in (False, True, "aax"):
         for tx, ty in [(64, 1), (32, 2), (16, 4), (8, 8), (64, 4), (32, 8)]:
             g = gpu.Lbm.from_config(cfg, aa=aa, vec=4)
             g.set_launch_shape(tx, ty)
@@ -155,7 +155,7 @@ def _check_stats(sg, so, u_bulk):
     assert np.abs(sg[:, 9] - so[:, 9]).max() <= 1e-6
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2), (33, 1), (512, 4)])
 def test_stats_parity(orc, gpu, aa, nx, vec):
     cfg = wl.small(nx=nx, ny=10, nz=6)
@@ -187,7 +187,7 @@ def test_set_macros_host_and_get_macros_host(orc, gpu):
     rho = rho * (1.0 + 0.01 * np.sin(np.arange(rho.size).reshape(rho.shape)))
     o.set_macros(rho, u)
     w = _weights(orc)
-    for aa in (False, True):
+    for aa in (False, True, "aax"):
         g = gpu.Lbm.from_config(cfg, aa=aa)
         g.set_macros_host(rho.astype(np.float32), u.astype(np.float32))
         assert _state_err(o, g, w) <= 5e-8
@@ -203,7 +203,7 @@ def test_set_macros_host_and_get_macros_host(orc, gpu):
 # ---------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json:configs[0]) at 1, 10, 100, 200 steps; config 2 at 100 steps
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 def test_cfg1_200_steps(orc, gpu, aa):
     cfg = wl.get("cfg1")
     o, g = _pair(orc, gpu, cfg, aa, 0)
@@ -265,7 +265,7 @@ def _gpu_err_vs(orc, gpu, cfg, seed, steps, aa):
 # north_star: "Over 100 steps, the macroscopic rho and u must satisfy max|delta| <= 1e-5 relative
 # to the bulk velocity".  Several seeds per config: the flow amplifies rounding differences, so
 # the margin is a property of the realisation, not only of the arithmetic.
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("seed", [12345, 1, 20220630, 987654321])
 def test_cfg1_100_steps_seeds(orc, gpu, aa, seed):
     cfg = wl.get("cfg1")
@@ -275,7 +275,7 @@ def test_cfg1_100_steps_seeds(orc, gpu, aa, seed):
     assert er <= tol and eu <= tol
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("seed", [12345, 1, 20220630])
 def test_cfg2_100_steps(orc, gpu, aa, seed):
     cfg = wl.get("cfg2")
@@ -285,7 +285,7 @@ def test_cfg2_100_steps(orc, gpu, aa, seed):
     assert er <= tol and eu <= tol
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 def test_cfg3_100_steps(orc, gpu, aa):
     """BASELINE.json:configs[2]: the first config with the Lalic-Mihailovic canopy (PAPER.md:L105-115,
     Eqs. 14-15) at full width, 512x128x256.  The oracle side is ~5 GB and runs once."""
@@ -348,13 +348,14 @@ def _subbox_check(orc, gpu, cfg, aa, boxes, presteps):
 
 
 @pytest.mark.parametrize("name,aa", [("cfg3", False), ("cfg3", True), ("cfg4", True), ("cfg5", True),
+                                     ("cfg3", "aax"), ("cfg5", "aax"), ("paper_abl_fine", "aax"),
                                      ("paper_channel", False), ("paper_channel", True),
                                      ("paper_abl_fine", False), ("paper_abl_fine", True)])
 def test_full_size_sampled_boxes(orc, gpu, name, aa):
     import torch
     cfg = wl.get(name)
     free, _ = torch.cuda.mem_get_info()
-    need = 76 * wl.n_cells(cfg) * (2 if aa else 3) * 1.05
+    need = 76 * wl.n_cells(cfg) * (2 if aa else 3) * 1.05          # populations + the get_state copy
     if free < need:
         pytest.skip(f"{name} needs {need / 2**30:.0f} GiB of device memory")
     nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
@@ -379,7 +380,7 @@ def test_full_size_sampled_boxes(orc, gpu, name, aa):
 # ---------------------------------------------------------------------------------------------
 # forced-equilibrium lid (NEXT #1)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("nx,vec", [(64, 4), (34, 2), (33, 1)])
 def test_forced_equilibrium_lid_parity(orc, gpu, aa, nx, vec):
     cfg = wl.small(nx=nx, ny=10, nz=6, top=wl.FORCED_EQ)
@@ -400,7 +401,7 @@ def test_forced_equilibrium_lid_parity(orc, gpu, aa, nx, vec):
 def test_couette_closed_form_on_gpu(gpu):
     """P14's closed form u_j = U (j + 1/2) / (ny + tau - 1/2) reached by the CUDA path itself."""
     ny, nu, U = 12, 0.2, 0.02
-    for aa in (False, True):
+    for aa in (False, True, "aax"):
         g = gpu.Lbm(8, ny, 4, nu, 0.0, flags=gpu.bc_flags("bounce_back", "forced_equilibrium", aa=aa))
         g.set_top_velocity([U, 0.0, 0.0])
         g.set_init(gpu.INIT_REST, 0.0, 0.0)
@@ -554,7 +555,7 @@ def test_forest_codes_need_a_geometry_handle(gpu):
 # ---------------------------------------------------------------------------------------------
 # CUDA-graph replay inside lbm_step: same kernels in the same order => bit-identical
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("every", [0, 1, 3, 4])
 def test_graph_replay_is_bit_identical(gpu, aa, every):
     import torch
@@ -591,10 +592,12 @@ def test_step_before_init_is_an_error(gpu):
 # ---------------------------------------------------------------------------------------------
 # lbm_set_state: checkpoint / restart, and pin P16 through the C ABI
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("t0", [4, 7])
 @pytest.mark.parametrize("solid", [False, True])
 def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
+    if aa == "aax" and solid:
+        pytest.skip("the x-balanced AA storage has no geometry variant")
     """get_state -> set_state(t) into a fresh handle -> step continues the run bit for bit."""
     import torch
     cfg = wl.small(nx=64, ny=10, nz=6)
@@ -623,7 +626,7 @@ def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
     assert torch.equal(ra, rb) and torch.equal(ua, ub)
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("t0", [0, 1])
 def test_p16_known_pi_neq_through_the_c_abi(orc, gpu, aa, t0):
     """Pin P16 (tests/test_oracle_pins.py) on the CUDA path: a periodic uniform state with a known

@@ -58,13 +58,13 @@ CONFIGS = {
     # BASELINE.json:configs[3]
     "cfg4": _cfg("cfg4", 1024, 256, 512, 1e-4, 0.1, 1.984e-7, 0.15, BOUNCE_BACK, FREE_SLIP,
                  dict(kind="lalic", h=32, LAI=2.0, eta_m=0.7), INIT_POWER_LAW, 0.08, 0.05,
-                 u_bulk=0.08, steps=1000, storage="aa", stats_every=1,
-                 note="large forest ABL, h=32, AA single array"),
+                 u_bulk=0.08, steps=1000, storage="aax", stats_every=1,
+                 note="large forest ABL, h=32, single-array AA pattern (x-balanced)"),
     # BASELINE.json:configs[4]
     "cfg5": _cfg("cfg5", 1536, 384, 1024, 1e-4, 0.1, 1.323e-7, 0.15, BOUNCE_BACK, FREE_SLIP,
                  dict(kind="lalic", h=48, LAI=2.0, eta_m=0.7), INIT_POWER_LAW, 0.08, 0.05,
-                 u_bulk=0.08, steps=500, storage="aa", stats_every=1,
-                 note="HBM-filling forest ABL, h=48, AA single array"),
+                 u_bulk=0.08, steps=500, storage="aax", stats_every=1,
+                 note="HBM-filling forest ABL, h=48, single-array AA pattern (x-balanced)"),
 }
 
 # The paper's own lattice shapes and cases.
