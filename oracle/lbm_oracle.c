@@ -12,13 +12,19 @@
  * shifted populations.  Readings of ambiguous passages are the ones tabulated in DESIGN.md
  * ("Readings", R1..) and cited at each site below.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): lattice identities, rest state, mass
- * conservation, Poiseuille, Taylor-Green, exact momentum increment, uniform-flow drag
- * recurrence, tau_total self-consistency, mirror equivalence, analytic plane statistics,
- * brute-force push streaming, z-mirror/translation symmetry, splitmix64 known answers, LAD
- * closed forms.  PARITY UNPINNED (no printed value or closed form in the paper fixes them; both
- * sides share the reading): (R4) no rho factor in the drag of Eq. 13, (R5) streamwise-only vs
- * vector drag direction, (R8) no forcing correction in Pi_neq.
+ * Pins (tests/test_oracle_pins.py, tests/test_paper_cases.py, -m "not gpu"): lattice identities (P0),
+ * rest state (P1), mass conservation (P2), Poiseuille (P3), Taylor-Green (P4), exact momentum
+ * increment (P5), uniform-flow drag recurrence (P6), tau_total self-consistency (P7), mirror
+ * equivalence (P8), analytic plane statistics (P9), z-mirror/translation symmetry (P12), brute-force
+ * push streaming (P13), Couette flow under the forced-equilibrium lid (P14), solid cells: brute-force
+ * push with random solids, solid layers == wall faces, mass (P15), the Pi_neq assembly inside the
+ * collision: relaxation of a known non-equilibrium part (P16), run-time removal of solids (P17),
+ * per-cell forest codes (P18), splitmix64 known answers, LAD closed forms, Table I / II / III numbers,
+ * the text's qualitative statements about the three ABL cases.
+ * PARITY UNPINNED (no printed value or closed form in the paper fixes them; both sides share the
+ * reading): (R4) no rho factor in the drag of Eq. 13, (R5) streamwise-only vs vector drag direction,
+ * (R8) no forcing correction in Pi_neq, (R9) Eq. 10 rather than Eq. 12 as printed where they differ
+ * (rho != 1), (R27) the bit layout of the forest code, (R28) f_eq(1, 0) in cells freed from a solid.
  *
  * Units: lattice units, dx = dt = 1, c = 1, c_s^2 = 1/3, filter width Delta = dx = 1.
  * Layout: cell = x + nx*(y + ny*z), x streamwise, y wall-normal, z spanwise; f[i*N + cell].

@@ -304,6 +304,9 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
 #pragma unroll
                         for (int k = 1; k < V; ++k) t[k] = r[k - 1];
                         stv<V>(rowp + c.x0, t);
+                    } else if constexpr (V == 4) {     // x0+1 alone, then the 8-byte aligned pair x0+2, x0+3
+                        rowp[c.x0 + 1] = r[0];
+                        *reinterpret_cast<float2 *>(rowp + c.x0 + 2) = make_float2(r[1], r[2]);
                     } else {
 #pragma unroll
                         for (int k = 0; k < V - 1; ++k) rowp[c.x0 + 1 + k] = r[k];
@@ -322,6 +325,9 @@ __device__ __forceinline__ void store_dir(const KParams &p, const Ctx &c, const 
                         for (int k = 0; k < V - 1; ++k) t[k] = r[k + 1];
                         t[V - 1] = rr;
                         stv<V>(rowp + c.x0, t);
+                    } else if constexpr (V == 4) {     // the 8-byte aligned pair x0, x0+1, then x0+2 alone
+                        *reinterpret_cast<float2 *>(rowp + c.x0) = make_float2(r[1], r[2]);
+                        rowp[c.x0 + 2] = r[3];
                     } else {
 #pragma unroll
                         for (int k = 1; k < V; ++k) rowp[c.x0 + k - 1] = r[k];
