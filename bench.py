@@ -269,6 +269,8 @@ def run_b200(args, cfg):
     if args.tma is not None:
         tm = [int(v) for v in args.tma.split(",")]
         sim.set_tma(tm[0], tm[1] if len(tm) > 1 else 0)
+    if args.sweep is not None:
+        sim.set_sweep(args.sweep)
     sim.init(cfg["seed"] + rank)
     sim.stats_accumulate(every)
     stream = torch.cuda.current_stream(dev)
@@ -513,6 +515,8 @@ def main():
     ap.add_argument("--shape", default=None, help="thread-block shape override TXxTY (tuning)")
     ap.add_argument("--tma", default=None,
                     help="A/B: step kinds on the TMA path, 'mode[,rows]' (bit 0 AA even, 1 AA odd, 2 pull)")
+    ap.add_argument("--sweep", type=int, choices=[0, 1], default=None,
+                    help="A/B: 0 = every step walks the lattice forward, 1 = alternating direction (default)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes (read+write) per step-kernel launch, from profiles/, to quote in the line")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

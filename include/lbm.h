@@ -278,6 +278,15 @@ int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
  * handles.  Call before or between lbm_step calls. */
 int lbm_set_tma(lbm_t *h, int mode, int rows);
 
+/* Sweep direction of the step kernel.  mode 1 (default): consecutive time steps walk the rows of
+ * the lattice in opposite directions, so that a step starts on the planes the previous step wrote
+ * last and finds them in the L2 cache (on lattices of a few hundred MB a sizeable part of the
+ * reads; on HBM-filling ones a per-mille effect).  mode 0: every step walks forward.  The order in
+ * which cells are visited has no effect on the result (the update of a cell needs
+ * the previous state of adjacent cells only): both modes are bit-identical.  The environment
+ * variable LBM_SWEEP=0|1 sets the default of new handles.  LBM_EINVAL for any other mode. */
+int lbm_set_sweep(lbm_t *h, int mode);
+
 /* Measurement hook (bench.py "roofline"): with on != 0, lbm_step brackets every step-kernel
  * launch (the fused S1-S8 kernel only, not the stage-2 reduction) with a pair of CUDA events on
  * the bound stream, up to 4096 launches between reads.  lbm_kernel_timing_read synchronises the

@@ -85,6 +85,11 @@ def lib():
         L.orc_mix64.argtypes = [C.c_uint64, C.c_uint64]
         L.orc_rand01.restype = C.c_double
         L.orc_rand01.argtypes = [C.c_uint64, C.c_uint64]
+        L.orc_tau_total_rows.restype = C.c_double
+        L.orc_tau_total_rows.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, dp]
+        L.orc_sgs_van_driest.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, dp]
+        L.orc_sgs_mean_shear.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.orc_set_sgs_rows.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_lad_shape.restype = C.c_double
         L.orc_lad_shape.argtypes = [C.c_double, C.c_double]
         L.orc_lad_profile.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp]
@@ -127,6 +132,24 @@ def guo(tau: float, u, F) -> np.ndarray:
 def tau_total(tau0: float, Csmag: float, rho: float, Pneq6) -> float:
     p = np.ascontiguousarray(Pneq6, dtype=np.float64)
     return lib().orc_tau_total(float(tau0), float(Csmag), float(rho), _dp(p))
+
+
+def tau_total_rows(tau0: float, C_j: float, Sbar_j: float, rho: float, Pneq6) -> float:
+    P = np.ascontiguousarray(Pneq6, dtype=np.float64)
+    return float(lib().orc_tau_total_rows(float(tau0), float(C_j), float(Sbar_j), float(rho), _dp(P)))
+
+
+def sgs_van_driest(ny: int, Cs: float, u_tau: float, nu: float, A_plus: float = 26.0, both_walls: bool = False):
+    out = np.zeros(ny)
+    lib().orc_sgs_van_driest(int(ny), float(Cs), float(u_tau), float(nu), float(A_plus), int(bool(both_walls)), _dp(out))
+    return out
+
+
+def sgs_mean_shear(stats, top_wall: bool = False):
+    st = np.ascontiguousarray(stats, dtype=np.float64)
+    out = np.zeros(st.shape[0])
+    lib().orc_sgs_mean_shear(_dp(st), int(st.shape[0]), int(bool(top_wall)), _dp(out))
+    return out
 
 
 def mix64(seed: int, ctr: int) -> int:
@@ -272,6 +295,18 @@ class Oracle:
         else:
             c = np.ascontiguousarray(codes, dtype=np.uint32).reshape(self.shape)
             lib().orc_set_forest_codes(self._h, c.ctypes.data_as(C.c_void_p), float(a_fm))
+
+    def set_sgs_rows(self, C_row=None, Sbar_row=None):
+        """Per-row SGS tables (other SGS models): C_smag,j and / or |<S>|_j; None, None = standard."""
+        ptrs = []
+        for a in (C_row, Sbar_row):
+            if a is None:
+                ptrs.append(None)
+            else:
+                a = np.ascontiguousarray(a, dtype=np.float64)
+                assert a.shape == (self.ny,)
+                ptrs.append(a.ctypes.data_as(C.c_void_p))
+        lib().orc_set_sgs_rows(self._h, ptrs[0], ptrs[1])
 
     def get_populations(self):
         f = np.zeros((19,) + self.shape)

@@ -19,12 +19,13 @@
  * push streaming (P13), Couette flow under the forced-equilibrium lid (P14), solid cells: brute-force
  * push with random solids, solid layers == wall faces, mass (P15), the Pi_neq assembly inside the
  * collision: relaxation of a known non-equilibrium part (P16), run-time removal of solids (P17),
- * per-cell forest codes (P18), splitmix64 known answers, LAD closed forms, Table I / II / III numbers,
+ * per-cell forest codes (P18), row-table SGS models (P19), splitmix64 known answers, LAD closed forms, Table I / II / III numbers,
  * the text's qualitative statements about the three ABL cases.
  * PARITY UNPINNED (no printed value or closed form in the paper fixes them; both sides share the
  * reading): (R4) no rho factor in the drag of Eq. 13, (R5) streamwise-only vs vector drag direction,
  * (R8) no forcing correction in Pi_neq, (R9) Eq. 10 rather than Eq. 12 as printed where they differ
- * (rho != 1), (R27) the bit layout of the forest code, (R28) f_eq(1, 0) in cells freed from a solid.
+ * (rho != 1), (R27) the bit layout of the forest code, (R28) f_eq(1, 0) in cells freed from a solid, (R29) which
+ * "other SGS models" (the paper names none).
  *
  * Units: lattice units, dx = dt = 1, c = 1, c_s^2 = 1/3, filter width Delta = dx = 1.
  * Layout: cell = x + nx*(y + ny*z), x streamwise, y wall-normal, z spanwise; f[i*N + cell].
@@ -73,6 +74,8 @@ typedef struct orc_s {
     unsigned char *solid; /* [N] 1 = solid (NEXT #2), NULL = none */
     uint32_t *fcode;      /* [N] per-cell forest code (NEXT #2), NULL = none; 0 = use lad[y] */
     double a_fm;          /* a_fm of Eq. 14 for the coded cells */
+    double *sgs_C;        /* [ny] per-row Smagorinsky constant C_smag,j (other SGS models), NULL = Csmag */
+    double *sgs_Sbar;     /* [ny] per-row mean-shear magnitude |<S>|_j (shear-improved model), NULL = 0 */
     double *fa, *fb;      /* [Q][N] */
     double *acc;          /* [ny][NSTAT] running sums */
     double *rowsum;       /* [nz][ny][NSTAT] scratch */
@@ -127,6 +130,66 @@ double orc_tau_total(double tau0, double Csmag, double rho, const double *Pneq)
                 2.0 * (Pneq[3] * Pneq[3] + Pneq[4] * Pneq[4] + Pneq[5] * Pneq[5]);
     double Qh = sqrt(QQ); /* Eq. 11 */
     return 0.5 * (tau0 + sqrt(tau0 * tau0 + 18.0 * sqrt(2.0) * Csmag * Qh / rho));
+}
+
+/* Other SGS models ("the standard Smagorinsky model is used ... A future work is to
+ * implement other SGS models").  The paper names none; two published eddy-
+ * viscosity closures that keep the local form of Eq. 10, nu_t = C Delta^2 x (a strain-rate measure),
+ * are restated here (reading R29).  With |S| the strain-rate magnitude that Eq. 10 takes
+ * from Pi_neq - Eq. 10 is tau_total = tau0 + 3 C |S| solved for tau_total, which fixes
+ * |S| = 3 Q^{1/2} / (sqrt(2) rho tau_total) -
+ *   wall-damped Smagorinsky (van Driest damping): nu_t = C_j |S|, C_j = C_smag D(y+_j)^2,
+ *       D = 1 - exp(-y+/A+): a per-row constant (orc_sgs_van_driest);
+ *   shear-improved Smagorinsky (Leveque, Toschi, Shao, Bertoglio 2007): nu_t = C (|S| - |<S>|),
+ *       never negative, <S> the mean shear - in a plane-homogeneous flow a per-row number
+ *       Sbar_j = |d<u>/dy| (orc_sgs_mean_shear).
+ * Both: tau_total = tau0 + 3 C_j (|S| - Sbar_j)_+.  While the bracket is positive this is the
+ * quadratic of Eq. 10 with tau0 replaced by tau0' = tau0 - 3 C_j Sbar_j,
+ *   tau_total = ( tau0' + sqrt( tau0'^2 + 18 sqrt(2) C_j Q^{1/2} / rho ) ) / 2,
+ * and the bracket is positive exactly when that root exceeds tau0; otherwise nu_t = 0 and
+ * tau_total = tau0.  C_j = C_smag, Sbar_j = 0 is Eq. 10 itself. */
+double orc_tau_total_rows(double tau0, double C_j, double Sbar_j, double rho, const double *Pneq)
+{
+    double QQ = Pneq[0] * Pneq[0] + Pneq[1] * Pneq[1] + Pneq[2] * Pneq[2] +
+                2.0 * (Pneq[3] * Pneq[3] + Pneq[4] * Pneq[4] + Pneq[5] * Pneq[5]);
+    double Qh = sqrt(QQ); /* Eq. 11 */
+    double tau0p = tau0 - 3.0 * C_j * Sbar_j;
+    double tau = 0.5 * (tau0p + sqrt(tau0p * tau0p + 18.0 * sqrt(2.0) * C_j * Qh / rho));
+    return (tau > tau0) ? tau : tau0;
+}
+
+/* van Driest damping of the Smagorinsky constant: C_j = Cs^2 [1 - exp(-y+_j / A+)]^2, y+_j =
+ * d_j u_tau / nu with d_j the distance of the cell centre j + 1/2 from the nearest no-slip wall
+ * (bottom wall only, or both walls of a channel). */
+void orc_sgs_van_driest(int ny, double Cs, double u_tau, double nu, double A_plus, int both_walls, double *C_out)
+{
+    for (int j = 0; j < ny; ++j) {
+        double d = j + 0.5;
+        if (both_walls && ny - d < d) d = ny - d;
+        double D = 1.0 - exp(-(d * u_tau / nu) / A_plus);
+        C_out[j] = Cs * Cs * D * D;
+    }
+}
+
+/* Mean-shear magnitude of a plane-averaged profile: |<S>| = sqrt(2 <S>:<S>) with <S>_xy =
+ * (1/2) d<u>/dy, <S>_yz = (1/2) d<w>/dy  =>  Sbar_j = sqrt( (d<u>/dy)^2 + (d<w>/dy)^2 ).
+ * Central differences between cell centres; at a no-slip wall the profile is extended with its
+ * mirror image of opposite sign (u = 0 on the face), at a free-slip or lid face with its mirror
+ * image (zero gradient).  stats = the [ny][10] table of orc_stats_read (columns 0 and 2).
+ * top_wall: 1 = no-slip wall at the top face, 0 = zero-gradient top. */
+void orc_sgs_mean_shear(const double *stats, int ny, int top_wall, double *Sbar_out)
+{
+    for (int j = 0; j < ny; ++j) {
+        double d[2];
+        for (int a = 0; a < 2; ++a) {
+            int col = a ? 2 : 0;
+            double below = (j > 0) ? stats[(j - 1) * NSTAT + col] : -stats[col];
+            double above = (j < ny - 1) ? stats[(j + 1) * NSTAT + col]
+                                        : (top_wall ? -stats[(ny - 1) * NSTAT + col] : stats[(ny - 1) * NSTAT + col]);
+            d[a] = 0.5 * (above - below);
+        }
+        Sbar_out[j] = sqrt(d[0] * d[0] + d[1] * d[1]);
+    }
 }
 
 /* Counter-based uniform generator in [0,1) shared by specification with the CUDA path
@@ -198,7 +261,7 @@ orc_t *orc_create(int nx, int ny, int nz, double nu, double Cs, const double *bo
 void orc_destroy(orc_t *o)
 {
     if (!o) return;
-    free(o->lad); free(o->solid); free(o->fcode); free(o->fa); free(o->fb); free(o->acc); free(o->rowsum);
+    free(o->lad); free(o->solid); free(o->fcode); free(o->sgs_C); free(o->sgs_Sbar); free(o->fa); free(o->fb); free(o->acc); free(o->rowsum);
     free(o);
 }
 
@@ -232,6 +295,21 @@ void orc_set_forest_codes(orc_t *o, const uint32_t *code /* [N] or NULL */, doub
     if (code) {
         o->fcode = (uint32_t *)malloc(sizeof(uint32_t) * o->N);
         memcpy(o->fcode, code, sizeof(uint32_t) * o->N);
+    }
+}
+
+/* Per-row SGS tables (see orc_tau_total_rows): C_j and / or Sbar_j, [ny] each; NULL, NULL restores
+ * the standard model of the paper. */
+void orc_set_sgs_rows(orc_t *o, const double *C_row, const double *Sbar_row)
+{
+    free(o->sgs_C); free(o->sgs_Sbar); o->sgs_C = NULL; o->sgs_Sbar = NULL;
+    if (C_row) {
+        o->sgs_C = (double *)malloc(sizeof(double) * o->ny);
+        memcpy(o->sgs_C, C_row, sizeof(double) * o->ny);
+    }
+    if (Sbar_row) {
+        o->sgs_Sbar = (double *)malloc(sizeof(double) * o->ny);
+        memcpy(o->sgs_Sbar, Sbar_row, sizeof(double) * o->ny);
     }
 }
 
@@ -385,7 +463,7 @@ static void macros_cell(const orc_t *o, long long cell, int y, const double *f, 
 }
 
 /* O7-O9: Smagorinsky relaxation time and forced BGK collision of one cell. */
-static void collide_cell(const orc_t *o, double rho, const double *u, const double *F,
+static void collide_cell(const orc_t *o, int y, double rho, const double *u, const double *F,
                          const double *Pi, const double *f, double *fstar)
 {
     /* Pi_neq = Pi - Pi_eq, Pi_eq = rho cs2 I + rho u u (reading R8) */
@@ -396,7 +474,11 @@ static void collide_cell(const orc_t *o, double rho, const double *u, const doub
     Pneq[3] = Pi[3] - rho * u[0] * u[1];
     Pneq[4] = Pi[4] - rho * u[1] * u[2];
     Pneq[5] = Pi[5] - rho * u[0] * u[2];
-    double tau = orc_tau_total(o->tau0, o->Csmag, rho, Pneq);   /* Eq. 12 */
+    double tau;
+    if (o->sgs_C || o->sgs_Sbar)                                 /* other SGS models (L307) */
+        tau = orc_tau_total_rows(o->tau0, o->sgs_C ? o->sgs_C[y] : o->Csmag, o->sgs_Sbar ? o->sgs_Sbar[y] : 0.0, rho, Pneq);
+    else
+        tau = orc_tau_total(o->tau0, o->Csmag, rho, Pneq);       /* Eq. 12 */
     double feq[Q], Fi[Q];
     orc_feq(rho, u, feq);                                        /* Eq. 3 */
     orc_guo(tau, u, F, Fi);                                      /* Eq. 4 with tau_total (R10) */
@@ -466,7 +548,7 @@ static void step_once(orc_t *o)
                     rs[6] += u[0] * u[1]; rs[7] += u[1] * u[2]; rs[8] += u[0] * u[2];
                     rs[9] += rho;
                 }
-                collide_cell(o, rho, u, F, Pi, f, fstar); /* Collide with the body force */
+                collide_cell(o, y, rho, u, F, Pi, f, fstar); /* Collide with the body force */
                 for (int i = 0; i < Q; ++i) o->fb[i * o->N + cell] = fstar[i];
             }
             if (sample)

@@ -42,7 +42,7 @@ SYMBOLS = [
     "lbm_set_top_velocity", "lbm_set_solid", "lbm_wall_friction_velocity",
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
-    "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma",
+    "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma", "lbm_set_sweep",
     "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14", "lbm_step_slab_begin", "lbm_step_slab_end",
 ]
 
@@ -101,6 +101,7 @@ def lib():
         L.lbm_set_reference_profile.argtypes = [vp, dp]
         L.lbm_get_reference_profile.argtypes = [vp, dp]
         L.lbm_set_tma.argtypes = [vp, C.c_int, C.c_int]
+        L.lbm_set_sweep.argtypes = [vp, C.c_int]
         L.lbm_time.argtypes = [vp]
         L.lbm_time.restype = C.c_longlong
         L.lbm_launch_count.argtypes = [vp]
@@ -410,6 +411,10 @@ class Lbm:
     def set_tma(self, mode: int, rows: int = 0):
         """Which step kinds stream through the TMA unit (bit 0 AA even, 1 AA odd, 2 pull); rows per tile."""
         _check(lib().lbm_set_tma(self._h, int(mode), int(rows)))
+
+    def set_sweep(self, mode: int):
+        """1 (default): consecutive steps walk the lattice in opposite directions (L2 reuse); 0: forward."""
+        _check(lib().lbm_set_sweep(self._h, int(mode)))
 
     def set_reference_profile(self, jx_ref=None):
         """Per-row momentum reference of the collision arithmetic (rounding only); None = 0."""

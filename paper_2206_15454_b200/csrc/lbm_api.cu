@@ -2,7 +2,7 @@
 // layout, kernel dispatch.  No torch types; the caller owns the device workspace and the stream.
 #include "../../include/lbm.h"
 #include "lbm_kernels.cuh"
-#include "lbm_tma.cuh"
+#include "lbm_launch.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -105,6 +105,7 @@ struct lbm_s {
     // pull) and rows per tile; maps of the two population arrays (box 256 x 1 x 1 x 1)
     bool tma_ok;
     int tma_mode, tma_rows;
+    int sweep;                  // 1: consecutive steps walk the rows in opposite directions (L2 reuse), 0: always forward
     CUtensorMap map_a, map_b;
     Layout L;
     char *ws;
@@ -308,6 +309,11 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     }
     h->pchunks = h->nchunk;
     if (h->tma_mode && nx / TMA_BOX > h->pchunks) h->pchunks = nx / TMA_BOX;
+    h->sweep = 1;
+    {
+        const char *e = getenv("LBM_SWEEP");        // A-B override: 0 = always forward
+        if (e && *e) h->sweep = (atoi(e) != 0) ? 1 : 0;
+    }
     h->zlo = h->halo ? 1 : 0; h->zhi = h->halo ? nz - 1 : nz;
     h->zg0 = h->halo ? -1 : 0; h->nzg = h->halo ? nz - 2 : nz;
     h->nfluid.assign(ny, (double)nx * (h->zhi - h->zlo));
@@ -690,64 +696,33 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
     }
 }
 
-template <int RM, int WM, bool S, int R>
-static cudaError_t launch_tma_r(lbm_s *h, const KParams &p0, const CUtensorMap &ms)
-{
-    static bool attr_set = false;
-    const int smem = (Q * R * TMA_BOX + Q * R) * 4;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(step_tma_kernel<RM, WM, S, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    KParams p = p0;
-    p.nchunk = h->nx / TMA_BOX;                   // tiles per row (make_ctx decomposes blockIdx with it)
-    dim3 block(TMA_TX, R), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / R * p.nchunk));
-    step_tma_kernel<RM, WM, S, R><<<grid, block, smem, h->stream>>>(p, ms);
-    h->launches++;
-    return cudaGetLastError();
-}
-template <int RM, int WM, bool S>
-static cudaError_t launch_tma(lbm_s *h, const KParams &p)
-{
-    // the map of the array this step reads (two-lattice: the roles swap every step)
-    const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
-    const CUtensorMap &ms = swapped ? h->map_b : h->map_a;
-    switch (h->tma_rows) {
-    case 4: return launch_tma_r<RM, WM, S, 4>(h, p, ms);
-    case 2: return launch_tma_r<RM, WM, S, 2>(h, p, ms);
-    default: return launch_tma_r<RM, WM, S, 1>(h, p, ms);
-    }
-}
-
-template <int V, bool S>
-static cudaError_t launch_step_vs(lbm_s *h, const KParams &p)
-{
-    if (V == 4 && h->tma_mode) {
-        if (!h->aa) { if (h->tma_mode & 4) return launch_tma<RD_PULL, WR_LOCAL, S>(h, p); }
-        else if ((h->t & 1) == 0) { if (h->tma_mode & 1) return launch_tma<RD_LOCAL, WR_LOCAL_OPP, S>(h, p); }
-        else if (h->tma_mode & 2) return launch_tma<RD_PULL_OPP, WR_PUSH, S>(h, p);
-    }
-    dim3 block(h->TX, h->TY), grid((unsigned)((long long)(p.z1 - p.z0) * h->ny / h->TY * h->nchunk));
-    if (h->mask) {
-        if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S, true><<<grid, block, 0, h->stream>>>(p);
-        else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S, true><<<grid, block, 0, h->stream>>>(p);
-        else step_kernel<V, RD_PULL_OPP, WR_PUSH, S, true><<<grid, block, 0, h->stream>>>(p);
-    } else if (!h->aa) step_kernel<V, RD_PULL, WR_LOCAL, S><<<grid, block, 0, h->stream>>>(p);
-    else if (h->aax && (h->t & 1) == 0) step_kernel<V, RD_XE, WR_XE, S><<<grid, block, 0, h->stream>>>(p);
-    else if (h->aax) step_kernel<V, RD_XO, WR_XO, S><<<grid, block, 0, h->stream>>>(p);
-    else if ((h->t & 1) == 0) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, S><<<grid, block, 0, h->stream>>>(p);
-    else step_kernel<V, RD_PULL_OPP, WR_PUSH, S><<<grid, block, 0, h->stream>>>(p);
-    h->launches++;
-    return cudaGetLastError();
-}
+// One launch of the fused step for the planes [p.z0, p.z1): the launchers live in their own
+// translation units (lbm_launch.cuh), one per (cells per thread, statistics, SGS row table).
 static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
 {
-    switch (h->V) {
-    case 4: return stats ? launch_step_vs<4, true>(h, p) : launch_step_vs<4, false>(h, p);
-    case 2: return stats ? launch_step_vs<2, true>(h, p) : launch_step_vs<2, false>(h, p);
-    default: return stats ? launch_step_vs<1, true>(h, p) : launch_step_vs<1, false>(h, p);
+    StepLaunch L;
+    L.TX = h->TX; L.TY = h->TY; L.nchunk = h->nchunk; L.nx = h->nx; L.ny = h->ny;
+    L.mask = h->mask; L.aa = h->aa; L.aax = h->aax; L.odd = (h->t & 1) != 0;
+    L.tma_mode = h->tma_mode; L.tma_rows = h->tma_rows;
+    // the map of the array this step reads (two-lattice: the roles swap every step)
+    const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
+    L.map = swapped ? &h->map_b : &h->map_a;
+    L.stream = h->stream;
+    const bool sgs = p.sgs != nullptr;
+    h->launches++;
+    if (h->V == 4 && h->tma_mode && !sgs) {
+        const cudaError_t e = stats ? launch_tma_t<true>(L, p) : launch_tma_t<false>(L, p);
+        if (e != cudaErrorNotSupported) return e;
     }
+#define LBM_GO(V) \
+    return stats ? (sgs ? launch_step_t<V, true, true>(L, p) : launch_step_t<V, true, false>(L, p)) \
+                 : (sgs ? launch_step_t<V, false, true>(L, p) : launch_step_t<V, false, false>(L, p));
+    switch (h->V) {
+    case 4: LBM_GO(4)
+    case 2: LBM_GO(2)
+    default: LBM_GO(1)
+    }
+#undef LBM_GO
 }
 
 static cudaError_t launch_stage2(lbm_s *h, int mode)
@@ -926,6 +901,7 @@ static KParams step_params(lbm_s *h, bool sample)
     KParams p = h->kp;
     if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }
     p.z0 = h->zlo; p.z1 = h->zhi;
+    p.rev = h->sweep ? (int)(h->t & 1) : 0;
     if (sample) {
         p.partial = reinterpret_cast<float *>(h->ws + h->L.partial);
         p.shift = (h->mask || h->halo) ? nullptr : reinterpret_cast<const float *>(h->ws + h->L.shift);
@@ -1192,6 +1168,16 @@ int lbm_set_tma(lbm_t *h, int mode, int rows)
     if (rows) h->tma_rows = rows;
     set_variant(h);
     return set_pchunks(h);
+}
+
+int lbm_set_sweep(lbm_t *h, int mode)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    if (mode != 0 && mode != 1) return fail(LBM_EINVAL, "mode must be 0 (forward) or 1 (alternating)");
+    DevGuard dg(h);
+    graph_drop(h);
+    h->sweep = mode;
+    return LBM_OK;
 }
 
 int lbm_set_graphs(lbm_t *h, int mode)

@@ -81,6 +81,8 @@ struct KParams {
     float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
     float Fbx, Fby, Fbz;        // body force density F_b
     const float *cda;           // [ny] C_D * a_j   (0 = not forest)
+    const float2 *sgs;          // [ny] per-row SGS table {tau0 - 3 C_j Sbar_j, 18 sqrt(2) C_j}; NULL = the
+                                // standard Smagorinsky model with the constants above (lbm_set_sgs_rows)
     const float *jref;          // [ny] r_j = J0_j / 12: per-row momentum reference (see mom_ref_shift)
     int bot, top, drag_vector;
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
@@ -103,6 +105,7 @@ struct KParams {
     double noise_amp;           // noise_frac * U_ref
     unsigned long long seed;
     int z0, z1;                 // z range of a launch (chunked host transfers; interior planes of a slab)
+    int rev;                    // 1 = the blocks walk the rows of the launch from the last to the first
     int zg0, nzg;               // z slab: global z of local plane 0 and global nz (init recipe only)
     int zv0, zv1;               // planes that hold the lattice proper ([1, nz-1) on a z slab: not the ghosts)
     long long zoff;             // element offset of plane z0 inside rho_in/u_in/rho_out/u_out
@@ -149,12 +152,22 @@ struct Ctx {
     bool edgeL, edgeR;  // lane has no x-neighbour lane on that side
 };
 
+// Sweep direction.  Blocks are scheduled in index order, so the rows a launch touches last are the
+// ones the 126 MB L2 still holds when the next launch starts.  Consecutive time steps walk the
+// lattice in opposite directions (p.rev alternates): a step starts on the planes the previous one
+// has just written and takes them from L2 instead of DRAM.  The order of the blocks has no effect
+// on the result (two-lattice: src and dst differ; in place: a block writes exactly what it read).
+__device__ __forceinline__ int block_index(const KParams &p)
+{
+    return p.rev ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
+}
+
 // `again`: recompute from laundered thread/block indices, so that the compiler does not keep the
 // first Ctx alive across the collision (register pressure of the AA odd step).
 template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0, bool again = false)
 {
     Ctx c;
-    int tx = threadIdx.x, ty = threadIdx.y, bx = blockIdx.x;
+    int tx = threadIdx.x, ty = threadIdx.y, bx = block_index(p);
     if (again) asm volatile("" : "+r"(tx), "+r"(ty), "+r"(bx));
     const int lane = (ty * blockDim.x + tx) & 31;
     // 1-D grid, the x chunks of a row are consecutive blocks (they run together, so the partial
@@ -659,8 +672,11 @@ __device__ __forceinline__ Cell moments(const KParams &p, const float (&g)[Q][V]
 //                       odd part   w_i  c.k,                 k = 3 w j + 3 (1-w/2) F.
 // The x-moving populations come in about the momentum reference (mom_ref_shift) and go out
 // plain: their odd part is built from j' = jx - J0 and ref_i is added back in the same sum.
-template <int V>
-__device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m, float r)
+// Row-table SGS models (lbm_set_sgs_rows; "other SGS models"): with a per-row
+// constant C_j and a per-row mean shear Sbar_j the closure nu_t = C_j (|S| - Sbar_j)_+ keeps the
+// closed form of Eq. 12 with tau0 replaced by tau0 - 3 C_j Sbar_j, clipped below at tau0.
+template <int V, bool SGS>
+__device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int k, const Cell &m, float r, int y)
 {
     const float ux = m.ux, uy = m.uy, uz = m.uz;
     const float third_drho = m.drho * (1.0f / 3.0f);
@@ -672,7 +688,13 @@ __device__ __forceinline__ void collide(const KParams &p, float (&g)[Q][V], int 
     const float nxz = m.Pxz - m.jx * uz;
     const float QQ = (nxx * nxx + nyy * nyy + nzz * nzz) + 2.0f * (nxy * nxy + nyz * nyz + nxz * nxz);
     const float Qh = sqrt_approx(QQ);                                                      // Eq. 11
-    const float tau = 0.5f * (p.tau0 + sqrt_approx(p.tau0sq + p.ksmag * Qh * m.inv_rho)); // Eq. 12
+    float tau;
+    if constexpr (SGS) {
+        const float2 sg = __ldg(p.sgs + y);
+        tau = fmaxf(0.5f * (sg.x + sqrt_approx(sg.x * sg.x + sg.y * Qh * m.inv_rho)), p.tau0);
+    } else {
+        tau = 0.5f * (p.tau0 + sqrt_approx(p.tau0sq + p.ksmag * Qh * m.inv_rho));          // Eq. 12
+    }
     const float w = rcp_approx(tau);
     const float omw = 1.0f - w;
     const float gp = 1.0f - 0.5f * w;                                           // Guo prefactor (R10)
@@ -830,7 +852,7 @@ template <int V, bool MASK> struct Bounds {
     static constexpr int minb = Occ<V>::minb;
 };
 
-template <int V, int RM, int WM, bool STATS, bool MASK>
+template <int V, int RM, int WM, bool STATS, bool MASK, bool SGS>
 __device__ __forceinline__ void step_body(const KParams &p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
@@ -867,7 +889,7 @@ __device__ __forceinline__ void step_body(const KParams &p)
             // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
             if (!MASK || !((solid_self<V>(S) >> k) & 1u)) stats_add(s, m);
         }
-        collide<V>(p, g, k, m, jr);
+        collide<V, SGS>(p, g, k, m, jr, c.y);
     }
     const Ctx c2 = (WM == WR_PUSH || WM == WR_XO) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
     if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
@@ -886,22 +908,22 @@ __device__ __forceinline__ void step_body(const KParams &p)
 // is built by blockflag_kernel whenever the geometry or the block shape changes).  The flag is one
 // byte per block, read before anything else; in sparse geometry almost every block takes the plain
 // path, so the instruction cache sees one body.
-template <int V, int RM, int WM, bool STATS, bool MASK = false>
+template <int V, int RM, int WM, bool STATS, bool MASK = false, bool SGS = false>
 __global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
 {
     if constexpr (MASK) {
-        const long long gb = (long long)blockIdx.x + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
+        const long long gb = (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
         if (__ldg(p.bflag + gb) == 0) {
-            step_body<V, RM, WM, STATS, false>(p);
+            step_body<V, RM, WM, STATS, false, SGS>(p);
             return;
         }
     }
-    step_body<V, RM, WM, STATS, MASK>(p);
+    step_body<V, RM, WM, STATS, MASK, SGS>(p);
 }
 
 // One thread per thread block of the step launch (block = tx_cells x ty rows, nchunk blocks per
 // row): flag = any bit of the dilated solid mask, or any coded forest cell, inside the block.
-__global__ void blockflag_kernel(const KParams p, int tx_cells, int ty, unsigned char *out, long long nblocks)
+static __global__ void blockflag_kernel(const KParams p, int tx_cells, int ty, unsigned char *out, long long nblocks)
 {
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nblocks) return;
@@ -1178,7 +1200,7 @@ __global__ void state_kernel(const KParams p, float *out)
 // grid = (ny, NSTAT), block = 256.  mode 0: accumulate; mode 1: prime the accumulation centre
 // shift[y][0..2] with the current plane means instead.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) stats_stage2_kernel(const float *__restrict__ partial, long long len,
+static __global__ void __launch_bounds__(256) stats_stage2_kernel(const float *__restrict__ partial, long long len,
                                                            double *acc, float *shift, int mode,
                                                            double inv_count, int *diverged)
 {

@@ -1,0 +1,32 @@
+// lbm_step_inst.cu — one explicit instantiation of the step-kernel launcher, selected by
+// -DLBM_V=<1|2|4> -DLBM_S=<0|1> -DLBM_G=<0|1> (cells per thread, fused statistics, row-table SGS):
+// 8 kernels per translation unit (5 storage modes + 3 geometry variants).  build.py compiles the
+// twelve of them in parallel.
+#include "lbm_launch.cuh"
+
+#if !defined(LBM_V) || !defined(LBM_S) || !defined(LBM_G)
+#error "compile with -DLBM_V=<1|2|4> -DLBM_S=<0|1> -DLBM_G=<0|1>"
+#endif
+
+namespace lbm {
+
+template <int V, bool STATS, bool SGS>
+cudaError_t launch_step_t(const StepLaunch &L, const KParams &p)
+{
+    dim3 block(L.TX, L.TY), grid((unsigned)((long long)(p.z1 - p.z0) * L.ny / L.TY * L.nchunk));
+    cudaStream_t st = L.stream;
+    if (L.mask) {
+        if (!L.aa) step_kernel<V, RD_PULL, WR_LOCAL, STATS, true, SGS><<<grid, block, 0, st>>>(p);
+        else if (!L.odd) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, true, SGS><<<grid, block, 0, st>>>(p);
+        else step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, true, SGS><<<grid, block, 0, st>>>(p);
+    } else if (!L.aa) step_kernel<V, RD_PULL, WR_LOCAL, STATS, false, SGS><<<grid, block, 0, st>>>(p);
+    else if (L.aax && !L.odd) step_kernel<V, RD_XE, WR_XE, STATS, false, SGS><<<grid, block, 0, st>>>(p);
+    else if (L.aax) step_kernel<V, RD_XO, WR_XO, STATS, false, SGS><<<grid, block, 0, st>>>(p);
+    else if (!L.odd) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, false, SGS><<<grid, block, 0, st>>>(p);
+    else step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, false, SGS><<<grid, block, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+template cudaError_t launch_step_t<LBM_V, (LBM_S != 0), (LBM_G != 0)>(const StepLaunch &, const KParams &);
+
+} // namespace lbm

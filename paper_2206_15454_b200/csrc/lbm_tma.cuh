@@ -22,18 +22,17 @@
 #pragma once
 #include <cuda.h>
 
-#include "lbm_kernels.cuh"
+#include "lbm_launch.cuh"
 
 namespace lbm {
 
-constexpr int TMA_BOX = 256;              // cells of a row segment = one TMA box (hardware max 256)
 constexpr int TMA_TX = TMA_BOX / 4;       // threads along x
 
-__constant__ signed char TMA_CX[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
-__constant__ signed char TMA_CY[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
-__constant__ signed char TMA_CZ[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
-__constant__ signed char TMA_OPP[Q] = {0, 2, 1, 4, 3, 6, 5, 8, 7, 10, 9, 12, 11, 14, 13, 16, 15, 18, 17};
-__constant__ signed char TMA_MIR[Q] = {0, 1, 2, 4, 3, 5, 6, 9, 10, 7, 8, 11, 12, 13, 14, 18, 17, 16, 15};
+static __constant__ signed char TMA_CX[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+static __constant__ signed char TMA_CY[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+static __constant__ signed char TMA_CZ[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+static __constant__ signed char TMA_OPP[Q] = {0, 2, 1, 4, 3, 6, 5, 8, 7, 10, 9, 12, 11, 14, 13, 16, 15, 18, 17};
+static __constant__ signed char TMA_MIR[Q] = {0, 1, 2, 4, 3, 5, 6, 9, 10, 7, 8, 11, 12, 13, 14, 18, 17, 16, 15};
 
 __device__ __forceinline__ uint32_t smem_addr(const void *p)
 {
@@ -219,7 +218,7 @@ step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc)
         mom_ref_shift<4>(g, k, jr);
         const Cell m = moments<4>(p, g, k, cda, jr);
         if constexpr (STATS) stats_add(s, m);
-        collide<4>(p, g, k, m, jr);
+        collide<4, false>(p, g, k, m, jr, c.y);
     }
     const Ctx c2 = (WM == WR_PUSH) ? make_ctx<4>(p, p.z0 * p.ny, true) : c;
     store_all<4, WM, false>(p, c2, g);

@@ -582,6 +582,44 @@ def test_graph_replay_is_bit_identical(gpu, aa, every):
     assert np.array_equal(sa, sb) and np.array_equal(ta, tb)
 
 
+# Sweep direction (lbm_set_sweep): the order in which the blocks visit the rows is free
+# (a cell needs the previous state of adjacent cells only) => bit-identical
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
+@pytest.mark.parametrize("solid", [False, True], ids=["plain", "boxes"])
+@pytest.mark.parametrize("nx", [64, 36, 33])
+def test_sweep_direction_is_bit_identical(gpu, aa, solid, nx):
+    import torch
+    if aa == "aax" and solid:
+        pytest.skip("the x-balanced AA storage has no geometry variant")
+    cfg = wl.small(nx=nx, ny=12, nz=10)
+    if solid:
+        m = np.zeros((cfg["nz"], cfg["ny"], cfg["nx"]), dtype=np.uint8)
+        m[2:5, 0:3, 5:9] = 1
+        m[7:9, 9:12, nx - 3:nx] = 1
+        cfg["solid"] = m
+    out = []
+    for mode in (0, 1):
+        g = gpu.Lbm.from_config(cfg, aa=aa)
+        g.set_sweep(mode)
+        g.set_graphs(0)
+        g.init(cfg["seed"])
+        g.stats_accumulate(2)
+        g.step(13)
+        st = g.get_state()
+        s, n = g.stats_read()
+        torch.cuda.synchronize()
+        out.append((st.cpu().numpy(), s, n))
+        g.close()
+    assert out[0][2] == out[1][2] == 7
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    with pytest.raises(gpu.LbmError):
+        g2 = gpu.Lbm.from_config(cfg, aa=aa)
+        try:
+            g2.set_sweep(2)
+        finally:
+            g2.close()
+
+
 def test_step_before_init_is_an_error(gpu):
     g = gpu.Lbm(8, 4, 4, 0.01, 0.1)
     with pytest.raises(gpu.LbmError) as e:

@@ -776,3 +776,156 @@ def test_p18_partial_forest_is_local(orc):
     part.set_populations(f)
     part.step(1)
     assert np.array_equal(part.get_populations(), fn)
+
+
+# ------------------------------------------------------------------------------------------
+# P19: row-table SGS models ("other SGS models"; reading R29)
+# ------------------------------------------------------------------------------------------
+
+def _tau_fixed_point(tau0, C, Sbar, rho, Qh, iters=200):
+    """The closure as it is DEFINED, iterated: tau = tau0 + 3 C max(|S| - Sbar, 0) with the strain
+    rate Eq. 10 takes from Pi_neq, |S| = 3 Q^{1/2} / (sqrt 2 rho tau).  (A contraction: the slope
+    3 C K / tau^2 is << 1 at these magnitudes.)  No closed form involved."""
+    tau = tau0
+    for _ in range(iters):
+        S = 3.0 * Qh / (np.sqrt(2.0) * rho * tau)
+        tau = tau0 + 3.0 * C * max(S - Sbar, 0.0)
+    return tau
+
+
+def test_p19_row_table_closure_against_its_definition(orc):
+    """orc_tau_total_rows is the closed-form root; the definition iterated to its fixed point must
+    give the same number, in the active branch, the clipped branch and at Sbar = 0, where it must
+    also equal the paper's Eq. 10 (orc_tau_total, pinned by P7)."""
+    rng = np.random.default_rng(19)
+    active = clipped = 0
+    for _ in range(200):
+        B = rng.normal(size=(3, 3))
+        A = 0.5 * (B + B.T) * 10 ** rng.uniform(-5, -2)
+        P6 = np.array([A[0, 0], A[1, 1], A[2, 2], A[0, 1], A[1, 2], A[0, 2]])
+        Qh = np.sqrt(np.sum(A * A))
+        rho = rng.uniform(0.9, 1.1)
+        tau0 = 3 * 10 ** rng.uniform(-4, -2) + 0.5
+        C = rng.uniform(0.0, 0.03)
+        S_now = 3.0 * Qh / (np.sqrt(2.0) * rho * tau0)
+        Sbar = rng.choice([0.0, rng.uniform(0, 0.8) * S_now, rng.uniform(1.05, 3.0) * S_now])
+        got = orc.tau_total_rows(tau0, C, Sbar, rho, P6)
+        want = _tau_fixed_point(tau0, C, Sbar, rho, Qh)
+        assert abs(got - want) <= 2e-15, (got, want)
+        if Sbar == 0.0:
+            assert got == orc.tau_total(tau0, C, rho, P6)
+        if got > tau0 * (1 + 1e-12):
+            active += 1
+            # the eddy viscosity it implies, nu_t = (tau - tau0)/3, is C (|S| - Sbar) at the final tau
+            S = 3.0 * Qh / (np.sqrt(2.0) * rho * got)
+            assert abs((got - tau0) / 3.0 - C * (S - Sbar)) <= 1e-15
+        else:
+            clipped += 1
+            assert got == tau0
+    assert active > 50 and clipped > 20
+
+
+@pytest.mark.parametrize("mode", ["damped", "shear_improved", "clipped"])
+def test_p19_row_tables_inside_the_collision(orc, mode):
+    """The P16 construction with per-row tables: on a periodic uniform state with a known Pi_neq = A
+    one step must relax f_neq by (1 - 1/tau_j), tau_j from the DEFINITION of the closure with that
+    row's C_j and Sbar_j - so the tables are read with the right row index (y, not x or z) and fed to
+    the right arguments."""
+    c, w, _, _ = orc.tables()
+    c = c.astype(float)
+    rng = np.random.default_rng(190)
+    nx, ny, nz = 4, 5, 3
+    B = rng.normal(size=(3, 3))
+    A = 0.5 * (B + B.T)
+    A -= np.trace(A) / 3 * np.eye(3)
+    A *= 2e-3
+    rho, u, nu, Cs = 1.03, np.array([0.09, -0.04, 0.03]), 2e-4, 0.12
+    tau0 = 3 * nu + 0.5
+    Qh = np.sqrt(np.sum(A * A))
+    S_now = 3.0 * Qh / (np.sqrt(2.0) * rho * tau0)
+    if mode == "damped":
+        C_row, Sbar_row = Cs ** 2 * np.array([0.0, 0.2, 0.5, 0.9, 1.0]), None
+    elif mode == "shear_improved":
+        C_row, Sbar_row = None, S_now * np.array([0.0, 0.3, 0.6, 0.9, 0.1])
+    else:
+        C_row, Sbar_row = Cs ** 2 * np.array([1.0, 0.5, 1.0, 2.0, 1.0]), S_now * np.array([1.5, 0.2, 4.0, 1.01, 0.0])
+    feq, fneq = _p16_state(w, c, rho, u, A)
+    o = orc.Oracle(nx, ny, nz, nu, Cs, (0, 0, 0), 0.0, None, _periodic_bc(orc))
+    o.set_sgs_rows(C_row, Sbar_row)
+    o.set_populations(np.broadcast_to((feq + fneq)[:, None, None, None], (19, nz, ny, nx)).copy())
+    o.step(1)
+    fs = o.get_populations()
+    taus = []
+    for j in range(ny):
+        Cj = Cs ** 2 if C_row is None else C_row[j]
+        Sj = 0.0 if Sbar_row is None else Sbar_row[j]
+        tau_j = _tau_fixed_point(tau0, Cj, Sj, rho, Qh)
+        taus.append(tau_j)
+        want = feq + (1 - 1 / tau_j) * fneq
+        assert np.abs(fs[:, :, j, :] - want[:, None, None]).max() <= 1e-15, j
+    assert len({round(t, 12) for t in taus}) >= 3          # the rows really differ
+    if mode == "clipped":
+        assert taus[0] == tau0 and taus[2] == tau0 and taus[1] > tau0
+    # back to the standard model: identical to a handle that never had tables
+    o.set_sgs_rows(None, None)
+    o.set_populations(np.broadcast_to((feq + fneq)[:, None, None, None], (19, nz, ny, nx)).copy())
+    o.step(1)
+    p = orc.Oracle(nx, ny, nz, nu, Cs, (0, 0, 0), 0.0, None, _periodic_bc(orc))
+    p.set_populations(np.broadcast_to((feq + fneq)[:, None, None, None], (19, nz, ny, nx)).copy())
+    p.step(1)
+    assert np.array_equal(o.get_populations(), p.get_populations())
+
+
+def test_p19_van_driest_and_mean_shear_tables(orc):
+    """Closed forms.  Damping: C_j = Cs^2 (1 - exp(-y+/A+))^2 with y+ = (j + 1/2) u_tau / nu; -> 0
+    at the wall like y+^2, -> Cs^2 far away; symmetric in a channel.  Mean shear: central
+    differences are exact for a parabola; the wall / symmetry extensions at the ends."""
+    ny, Cs, ut, nu, Ap = 40, 0.1, 2.5e-3, 2e-4, 26.0
+    C1 = orc.sgs_van_driest(ny, Cs, ut, nu, Ap, both_walls=False)
+    yp = (np.arange(ny) + 0.5) * ut / nu
+    assert np.allclose(C1, Cs ** 2 * (1 - np.exp(-yp / Ap)) ** 2, rtol=1e-14, atol=0)
+    assert C1[0] < 0.06 * Cs ** 2 and np.all(np.diff(C1) > 0) and abs(C1[-1] / Cs ** 2 - 1) < 1e-6
+    C2 = orc.sgs_van_driest(ny, Cs, ut, nu, Ap, both_walls=True)
+    assert np.array_equal(C2, C2[::-1]) and np.array_equal(C2[: ny // 2], C1[: ny // 2])
+    # channel parabola u = 4 U eta (1 - eta), eta = (j + 1/2)/ny, walls at both faces
+    U = 0.05
+    y = np.arange(ny) + 0.5
+    st = np.zeros((ny, 10))
+    st[:, 0] = 4 * U * (y / ny) * (1 - y / ny)
+    st[:, 2] = 0.5 * st[:, 0]                                   # a spanwise mean flow too
+    S = orc.sgs_mean_shear(st, top_wall=True)
+    dudy = 4 * U / ny * (1 - 2 * y / ny)
+    want = np.abs(dudy) * np.sqrt(1 + 0.25)
+    assert np.allclose(S[1:-1], want[1:-1], rtol=1e-12, atol=1e-18)
+    # wall rows: mirror image of opposite sign => (u_1 + u_0)/2 per unit length
+    assert np.isclose(S[0], 0.5 * (st[1, 0] + st[0, 0]) * np.sqrt(1.25), rtol=1e-13)
+    assert np.isclose(S[-1], S[0], rtol=1e-12)
+    # zero-gradient top: (u_{ny-1} - u_{ny-2})/2
+    S2 = orc.sgs_mean_shear(st, top_wall=False)
+    assert np.isclose(S2[-1], 0.5 * abs(st[-1, 0] - st[-2, 0]) * np.sqrt(1.25), rtol=1e-12)
+    assert np.array_equal(S2[:-1], S[:-1])
+
+
+def test_p19_wall_damping_lowers_the_eddy_viscosity_near_the_wall_only(orc):
+    """A short forced half-channel run, standard against damped: the two must differ near the wall
+    (where C_j is reduced) and the damped run must stay stable, conserve mass, and coincide with the
+    standard model when every C_j = Cs^2 (bit for bit: same arithmetic path apart from the clip)."""
+    cfg = wl.small(16, 12, 8, Cs=0.17, forest_rows=0)
+    def run(C_row):
+        o = orc.Oracle.from_config(cfg)
+        o.init_from_config(cfg)
+        if C_row is not None:
+            o.set_sgs_rows(C_row, None)
+        m0 = o.get_populations().sum()
+        o.step(30)
+        f = o.get_populations()
+        assert abs(f.sum() - m0) <= 1e-12 * m0
+        return f
+    f_std = run(None)
+    f_same = run(np.full(12, 0.17 ** 2))
+    assert np.abs(f_same - f_std).max() <= 1e-16                 # clip never active: same root
+    C = orc.sgs_van_driest(12, 0.17, 0.004, cfg["nu"], 26.0)
+    assert C[0] < 0.01 * 0.17 ** 2 and C[-1] > 0.6 * 0.17 ** 2
+    f_damp = run(C)
+    d = np.abs(f_damp - f_std).max(axis=(0, 1, 3))               # per row y
+    assert d[0] > 5 * d[-1] > 0 and d[0] == d.max()              # largest where C_j is cut most
