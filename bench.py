@@ -523,6 +523,8 @@ def main():
     ap.add_argument("--boxes", action="store_true",
                     help="geometry handle with the paper's turbulence-trip boxes in place (PAPER.md:L226): "
                          "times the geometry variants of the kernels")
+    ap.add_argument("--geometry", action="store_true",
+                    help="geometry handle (LBM_SOLID_MASK) with an all-fluid mask: the cost of the per-block flag alone")
     ap.add_argument("--sharded", action="store_true",
                     help="one lattice cut into N z slabs with a halo exchange per step (opt-in)")
     args = ap.parse_args()
@@ -542,6 +544,11 @@ def main():
         from paper_2206_15454_b200.run_paper_cases import trip_boxes
         cfg["solid"] = trip_boxes(cfg)
         cfg["note"] += ", trip boxes in place (geometry kernels)"
+    if args.geometry:
+        cfg["geometry"] = True
+        cfg["note"] += ", geometry handle with an all-fluid mask"
+    if (args.boxes or args.geometry) and cfg["storage"] == "aax":
+        cfg["storage"] = "aa"          # the geometry variants exist for the two-lattice and AA storage
     if args.impl == "reference":
         return run_reference(args, cfg)
     if args.sharded:

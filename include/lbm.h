@@ -278,6 +278,32 @@ int lbm_set_launch_shape(lbm_t *h, int tx, int ty);
  * handles.  Call before or between lbm_step calls. */
 int lbm_set_tma(lbm_t *h, int mode, int rows);
 
+/* Other SGS models ("the standard Smagorinsky model is used ... A future work is to
+ * implement other SGS models"; reading R29).  Per-row tables generalise
+ * Eq. 10 (L83) to nu_t = C_j (|S| - Sbar_j), never negative, i.e.
+ *   tau_total = max( tau0, ( t_j + sqrt( t_j^2 + 18 sqrt(2) C_j Q^{1/2} / rho ) ) / 2 ),  t_j = tau0 - 3 C_j Sbar_j,
+ * which covers the wall-damped Smagorinsky model (C_j from lbm_sgs_van_driest, Sbar = 0) and the
+ * shear-improved Smagorinsky model (Sbar_j = magnitude of the mean shear, lbm_sgs_mean_shear of a
+ * statistics table; the caller refreshes it as the mean profile develops).  csmag_row_host,
+ * sbar_row_host: [ny] doubles, host memory, read during the call; NULL csmag_row = Cs^2 of
+ * lbm_create on every row, NULL sbar_row = 0; both NULL restores the standard model.  Entries must be
+ * finite and >= 0 (LBM_EINVAL).  Costs 0 bytes per cell (one 8-byte table entry per row); handles
+ * with tables run the SGS variants of the step kernel, never the TMA path.  Call after lbm_bind
+ * (LBM_ESTATE otherwise), before or between lbm_step calls. */
+int lbm_set_sgs_rows(lbm_t *h, const double *csmag_row_host, const double *sbar_row_host);
+
+/* van Driest wall damping of the Smagorinsky constant: csmag_row_out[j] = Cs^2 (1 - exp(-y+_j/A+))^2,
+ * y+_j = d_j u_tau / nu, d_j = distance of the cell centre j + 1/2 to the bottom wall face (to the
+ * nearer of the two wall faces with both_walls != 0); A+ is usually 26.  Host only. */
+int lbm_sgs_van_driest(int ny, double Cs, double u_tau, double nu, double A_plus, int both_walls,
+                       double *csmag_row_out);
+
+/* Mean-shear magnitude of a statistics table ([ny][10] of lbm_stats_read, columns <u> and <w>):
+ * sbar_row_out[j] = sqrt((d<u>/dy)^2 + (d<w>/dy)^2), central differences between cell centres; the
+ * profile continues past a no-slip wall face as its odd image (bottom always; top with top_wall !=
+ * 0) and past a free-slip / lid face as its even image.  Host only. */
+int lbm_sgs_mean_shear(const double *stats_host, int ny, int top_wall, double *sbar_row_out);
+
 /* Sweep direction of the step kernel.  mode 1 (default): consecutive time steps walk the rows of
  * the lattice in opposite directions, so that a step starts on the planes the previous step wrote
  * last and finds them in the L2 cache (on lattices of a few hundred MB a sizeable part of the

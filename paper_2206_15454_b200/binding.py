@@ -43,6 +43,7 @@ SYMBOLS = [
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
     "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma", "lbm_set_sweep",
+    "lbm_set_sgs_rows", "lbm_sgs_van_driest", "lbm_sgs_mean_shear",
     "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14", "lbm_step_slab_begin", "lbm_step_slab_end",
 ]
 
@@ -102,6 +103,9 @@ def lib():
         L.lbm_get_reference_profile.argtypes = [vp, dp]
         L.lbm_set_tma.argtypes = [vp, C.c_int, C.c_int]
         L.lbm_set_sweep.argtypes = [vp, C.c_int]
+        L.lbm_set_sgs_rows.argtypes = [vp, vp, vp]
+        L.lbm_sgs_van_driest.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp]
+        L.lbm_sgs_mean_shear.argtypes = [vp, C.c_int, C.c_int, vp]
         L.lbm_time.argtypes = [vp]
         L.lbm_time.restype = C.c_longlong
         L.lbm_launch_count.argtypes = [vp]
@@ -194,6 +198,23 @@ def stats_from_raw(raw: np.ndarray, count: float, centre=None) -> np.ndarray:
     return out
 
 
+def sgs_van_driest(ny: int, Cs: float, u_tau: float, nu: float, A_plus: float = 26.0, both_walls: bool = False) -> np.ndarray:
+    """C_smag per row with van Driest wall damping (lbm_sgs_van_driest)."""
+    out = np.zeros(int(ny))
+    _check(lib().lbm_sgs_van_driest(int(ny), float(Cs), float(u_tau), float(nu), float(A_plus),
+                                    int(bool(both_walls)), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def sgs_mean_shear(stats: np.ndarray, top_wall: bool = False) -> np.ndarray:
+    """Mean-shear magnitude per row of a statistics table (lbm_sgs_mean_shear)."""
+    st = np.ascontiguousarray(stats, dtype=np.float64)
+    out = np.zeros(st.shape[0])
+    _check(lib().lbm_sgs_mean_shear(C.c_void_p(st.ctypes.data), int(st.shape[0]), int(bool(top_wall)),
+                                    C.c_void_p(out.ctypes.data)))
+    return out
+
+
 def mix64(seed: int, ctr: int) -> int:
     return int(lib().lbm_mix64(C.c_uint64(seed), C.c_uint64(ctr)))
 
@@ -234,7 +255,10 @@ class Lbm:
     """One simulation handle.  Arrays: rho (nz, ny, nx), u (3, nz, ny, nx), float32."""
 
     def __init__(self, nx, ny, nz, nu, Cs, body_force=(0.0, 0.0, 0.0), Cd=0.0, lad=None, flags=0,
-                 device="cuda:0", stream=None):
+                 device="cuda:0", stream=None, guard: int = 0):
+        """guard > 0 (debugging aid): the workspace is allocated with `guard` extra bytes on either
+        side, filled with a byte pattern; guard_intact() tells whether any kernel wrote outside the
+        workspace it was given."""
         import torch
 
         if not torch.cuda.is_available():
@@ -257,11 +281,15 @@ class Lbm:
                             bf.ctypes.data_as(dp), float(Cd), ladp, self.flags))
         self._h = h
         nbytes = workspace_bytes(self.nx, self.ny, self.nz, self.flags)
+        self._guard = (int(guard) + 255) // 256 * 256
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self._ws = torch.empty(nbytes + 256 + 2 * self._guard, dtype=torch.uint8, device=self.device)
+            if self._guard:
+                self._ws.fill_(0xA5)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         base = self._ws.data_ptr()
-        aligned = (base + 255) // 256 * 256
+        aligned = (base + self._guard + 255) // 256 * 256
+        self._ws_span = (aligned - base, nbytes)
         _check(L.lbm_bind(self._h, C.c_void_p(aligned), C.c_size_t(nbytes), C.c_void_p(self._stream.cuda_stream)))
 
     @classmethod
@@ -283,6 +311,15 @@ class Lbm:
         if cfg.get("forest_cells") is not None:
             s.set_forest_codes(*forest_codes_from_spec(cfg["forest_cells"], s.shape))
         return s
+
+    def guard_intact(self) -> bool:
+        """True if every byte of the workspace allocation outside the bound range still holds the
+        fill pattern (only meaningful for handles created with guard > 0)."""
+        import torch
+
+        torch.cuda.synchronize(self.device)
+        off, n = self._ws_span
+        return bool((self._ws[:off] == 0xA5).all()) and bool((self._ws[off + n:] == 0xA5).all())
 
     def close(self):
         h = getattr(self, "_h", None)
@@ -411,6 +448,20 @@ class Lbm:
     def set_tma(self, mode: int, rows: int = 0):
         """Which step kinds stream through the TMA unit (bit 0 AA even, 1 AA odd, 2 pull); rows per tile."""
         _check(lib().lbm_set_tma(self._h, int(mode), int(rows)))
+
+    def set_sgs_rows(self, csmag_row=None, sbar_row=None):
+        """Per-row SGS tables (other SGS models): C_smag,j and / or mean shear |<S>|_j; None, None = standard."""
+        keep, ptrs = [], []
+        for a in (csmag_row, sbar_row):
+            if a is None:
+                ptrs.append(None)
+            else:
+                a = np.ascontiguousarray(a, dtype=np.float64)
+                if a.shape != (self.ny,):
+                    raise ValueError(f"SGS row table must have shape ({self.ny},)")
+                keep.append(a)
+                ptrs.append(C.c_void_p(a.ctypes.data))
+        _check(lib().lbm_set_sgs_rows(self._h, ptrs[0], ptrs[1]))
 
     def set_sweep(self, mode: int):
         """1 (default): consecutive steps walk the lattice in opposite directions (L2 reuse); 0: forward."""

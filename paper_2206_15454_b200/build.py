@@ -62,11 +62,27 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS + [os.path.abspath(__file__)])
 
 
+def _stale(obj: str, src: str) -> bool:
+    """An object is rebuilt when its source, a header it includes or this script is newer."""
+    o = os.path.join(OBJ, obj)
+    if not os.path.exists(o):
+        return True
+    deps = [os.path.join(CSRC, src), os.path.join(CSRC, "lbm_kernels.cuh"), os.path.join(CSRC, "lbm_launch.cuh"),
+            os.path.abspath(__file__)]
+    if src == "lbm_tma_inst.cu":
+        deps.append(os.path.join(CSRC, "lbm_tma.cuh"))
+    if src == "lbm_api.cu":
+        deps.append(os.path.join(ROOT, "include", "lbm.h"))
+    t = os.path.getmtime(o)
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or needs_build()):
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     nvcc = nvcc_path()
+    todo = [u for u in units() if force or _stale(u[0], u[1])]
 
     def compile_one(u):
         obj, src, defs = u
@@ -75,9 +91,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         r = subprocess.run(cmd, capture_output=True, text=True)
         return obj, cmd, r
 
-    jobs = max(1, min(len(units()), os.cpu_count() or 1))
+    jobs = max(1, min(len(todo), os.cpu_count() or 1))
     with ThreadPoolExecutor(jobs) as ex:
-        results = list(ex.map(compile_one, units()))
+        results = list(ex.map(compile_one, todo))
     for obj, cmd, r in results:
         if verbose:
             print(" ".join(cmd), file=sys.stderr)

@@ -50,7 +50,7 @@ static size_t staging_budget()
 }
 
 struct Layout {
-    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, flag, solid, solid_nb, fidx, ftab, frow, bflag, staging, total;
+    size_t pops, pops2, partial, acc, shift, cda, uprof, jref, sgs, flag, solid, solid_nb, fidx, ftab, frow, bflag, staging, total;
     int stage_planes;
 };
 
@@ -68,6 +68,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     L.cda = off; off = align_up(off + (size_t)ny * 4, 256);
     L.uprof = off; off = align_up(off + (size_t)ny * 4, 256);
     L.jref = off; off = align_up(off + (size_t)ny * 4, 256);
+    L.sgs = off; off = align_up(off + (size_t)ny * 8, 256);
     L.flag = off; off += 256;
     L.solid = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
     L.solid_nb = off; if (mask) off = align_up(off + (size_t)((nx + 31) / 32) * ny * nz * 4, 256);
@@ -95,6 +96,7 @@ struct lbm_s {
     bool aa, aax, drag_vector, mask, halo;   // aax: the x-balanced variant of the AA pattern (aa is set too)
     bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
     bool forest_codes;          // per-cell forest codes installed (geometry handles)
+    bool sgs_rows;              // per-row SGS table installed (lbm_set_sgs_rows)
     bool slab_open, slab_sample; // between lbm_step_slab_begin and _end; that step samples
     int zg0, nzg;               // z slab: global plane of local plane 0, global nz
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
@@ -325,6 +327,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->g_launches = 0; h->g_samples = 0;
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
     h->forest_codes = false;
+    h->sgs_rows = false;
     h->slab_open = false; h->slab_sample = false;
     set_variant(h);
     *out = h;
@@ -364,6 +367,7 @@ static void fill_params(lbm_s *h)
     p.Fbx = (float)h->Fb[0]; p.Fby = (float)h->Fb[1]; p.Fbz = (float)h->Fb[2];
     p.cda = reinterpret_cast<const float *>(h->ws + h->L.cda);
     p.jref = reinterpret_cast<const float *>(h->ws + h->L.jref);
+    p.sgs = h->sgs_rows ? reinterpret_cast<const float2 *>(h->ws + h->L.sgs) : nullptr;
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
     {
         // lid populations f_eq,i(1, U_top) - w_i (Eq. 3) of the five directions with c_y = -1
@@ -448,6 +452,7 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
     CU_TRY(cudaMemsetAsync(h->ws + h->L.shift, 0, (size_t)h->ny * 16, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.flag, 0, 256, h->stream));
     CU_TRY(cudaMemsetAsync(h->ws + h->L.jref, 0, (size_t)h->ny * 4, h->stream));
+    h->sgs_rows = false; h->kp.sgs = nullptr;
     CU_TRY(cudaMemsetAsync(h->ws + h->L.partial, 0, h->L.acc - h->L.partial, h->stream));
     if (h->mask) {
         const size_t mbytes = (size_t)((h->nx + 31) / 32) * h->ny * h->nz * 4;
@@ -1168,6 +1173,63 @@ int lbm_set_tma(lbm_t *h, int mode, int rows)
     if (rows) h->tma_rows = rows;
     set_variant(h);
     return set_pchunks(h);
+}
+
+// Row-table SGS models: tau_total = max(tau0, (t + sqrt(t^2 + 18 sqrt(2) C_j Q^{1/2} / rho)) / 2) with
+// t = tau0 - 3 C_j Sbar_j; the table holds {t, 18 sqrt(2) C_j} per row.
+int lbm_set_sgs_rows(lbm_t *h, const double *csmag_row_host, const double *sbar_row_host)
+{
+    if (!h) return fail(LBM_EINVAL, "handle is NULL");
+    DevGuard dg(h);
+    if (!h->bound) return fail(LBM_ESTATE, "lbm_set_sgs_rows before lbm_bind");
+    graph_drop(h);
+    if (!csmag_row_host && !sbar_row_host) {
+        h->sgs_rows = false; h->kp.sgs = nullptr;
+        return LBM_OK;
+    }
+    const double tau0 = 3.0 * h->nu + 0.5;
+    std::vector<float> tab((size_t)h->ny * 2);
+    for (int j = 0; j < h->ny; ++j) {
+        const double C = csmag_row_host ? csmag_row_host[j] : h->Cs * h->Cs;
+        const double S = sbar_row_host ? sbar_row_host[j] : 0.0;
+        if (!(C >= 0.0) || !std::isfinite(C)) return fail(LBM_EINVAL, "csmag_row[%d] must be >= 0", j);
+        if (!(S >= 0.0) || !std::isfinite(S)) return fail(LBM_EINVAL, "sbar_row[%d] must be >= 0", j);
+        tab[2 * j] = (float)(tau0 - 3.0 * C * S);
+        tab[2 * j + 1] = (float)(18.0 * std::sqrt(2.0) * C);
+    }
+    CU_TRY(cudaMemcpyAsync(h->ws + h->L.sgs, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));     // tab is a local vector
+    h->sgs_rows = true;
+    h->kp.sgs = reinterpret_cast<const float2 *>(h->ws + h->L.sgs);
+    return LBM_OK;
+}
+
+int lbm_sgs_van_driest(int ny, double Cs, double u_tau, double nu, double A_plus, int both_walls, double *csmag_row_out)
+{
+    if (ny < 1 || !csmag_row_out) return fail(LBM_EINVAL, "bad arguments");
+    if (!(Cs >= 0.0) || !(u_tau >= 0.0) || !(nu > 0.0) || !(A_plus > 0.0)) return fail(LBM_EINVAL, "Cs, u_tau >= 0 and nu, A_plus > 0 are required");
+    for (int j = 0; j < ny; ++j) {
+        double dist = j + 0.5;                                  // cell centre to the bottom wall face
+        if (both_walls) dist = std::fmin(dist, (double)ny - dist);
+        const double damp = -std::expm1(-dist * u_tau / (nu * A_plus));   // 1 - exp(-y+/A+)
+        csmag_row_out[j] = Cs * Cs * damp * damp;
+    }
+    return LBM_OK;
+}
+
+int lbm_sgs_mean_shear(const double *stats, int ny, int top_wall, double *sbar_row_out)
+{
+    if (!stats || ny < 1 || !sbar_row_out) return fail(LBM_EINVAL, "bad arguments");
+    auto prof = [&](int j, int col) {       // profile extended past the faces: odd image at a wall, even otherwise
+        if (j < 0) return -stats[col];
+        if (j >= ny) return (top_wall ? -1.0 : 1.0) * stats[(size_t)(ny - 1) * NSTAT + col];
+        return stats[(size_t)j * NSTAT + col];
+    };
+    for (int j = 0; j < ny; ++j) {
+        const double du = 0.5 * (prof(j + 1, 0) - prof(j - 1, 0)), dw = 0.5 * (prof(j + 1, 2) - prof(j - 1, 2));
+        sbar_row_out[j] = std::hypot(du, dw);
+    }
+    return LBM_OK;
 }
 
 int lbm_set_sweep(lbm_t *h, int mode)

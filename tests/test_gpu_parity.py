@@ -2,9 +2,9 @@
 
 Every test runs the CUDA library (paper_2206_15454_b200) and the fp64 CPU oracle (oracle/) on the
 same seeded inputs and compares element by element.  Tolerances:
-  * macroscopic rho, u after <= 100 steps: max|delta| <= 1e-5 * u_bulk (BASELINE.json:north_star
-    fixes the bound "over 100 steps"); at 200 steps, where the seeded grid-scale noise has
-    amplified the fp32 rounding differences further, 4e-5 * u_bulk (DESIGN.md "Tolerances");
+  * macroscopic rho, u after 1, 10, 100 and 200 steps: max|delta| <= 1e-5 * u_bulk
+    (BASELINE.json:north_star fixes the bound "over 100 steps"; SURVEY P10 lists step 200 at the
+    same bound, and it holds there too);
   * one-step / few-step population checks: 2e-7 absolute (fp32 rounding of O(0.05) deviations
     from the weights, a few operations deep), far below any indexing or boundary-link mistake,
     which shows up at the 1e-3 level.
@@ -216,7 +216,9 @@ def test_cfg1_200_steps(orc, gpu, aa):
         g.step(target - done)
         done = target
         er, eu = _macro_err(o, g)
-        tol_t = tol if target <= 100 else 4.0 * tol
+        # north_star states the bound over 100 steps; with the momentum reference of the collision
+        # arithmetic step 200 meets the same bound (measured 8e-8)
+        tol_t = tol
         print(f"cfg1 {g.variant} step {target}: max|drho|={er:.3e} max|du|={eu:.3e} (tol {tol_t:.1e})")
         assert er <= tol_t and eu <= tol_t
     so, no = o.stats_read()
@@ -620,6 +622,98 @@ def test_sweep_direction_is_bit_identical(gpu, aa, solid, nx):
             g2.close()
 
 
+# ---------------------------------------------------------------------------------------------
+# Memory safety and races without compute-sanitizer (closed on this GPU pool):
+#  * guard bands: the workspace sits between two regions filled with a byte pattern; no kernel of
+#    any call may change a byte of them (an out-of-range store of a boundary / wrap / halo index
+#    lands there or faults);
+#  * run-to-run bit identity: a data race between lanes or blocks of the in-place AA update (the
+#    masked push path mixes vector and element stores to neighbouring lanes' cells) shows as a
+#    result that depends on scheduling.
+# ---------------------------------------------------------------------------------------------
+_GUARD_SHAPES = [(64, 12, 10, 4), (36, 7, 5, 4), (34, 5, 3, 2), (33, 3, 4, 1), (4, 1, 1, 4), (1, 5, 1, 1), (256, 4, 3, 4)]
+
+
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
+@pytest.mark.parametrize("kind", ["plain", "solid", "slab"])
+def test_guard_bands_stay_untouched(gpu, aa, kind):
+    import torch
+    if kind != "plain" and aa == "aax":
+        pytest.skip("the x-balanced AA storage has no geometry / slab variant")
+    if kind == "slab" and aa:
+        pytest.skip("z slabs use the two-lattice storage")
+    for nx, ny, nz, vec in _GUARD_SHAPES:
+        if kind == "slab" and nz < 3:
+            continue
+        for bottom, top in BCS + [(wl.BOUNCE_BACK, wl.FORCED_EQ)]:
+            cfg = wl.small(nx=nx, ny=ny, nz=nz, bottom=bottom, top=top, forest_rows=min(3, ny))
+            flags = gpu.bc_flags(bottom, top, aa=aa, vec=vec, solid=(kind == "solid"), halo=(kind == "slab"))
+            g = gpu.Lbm(nx, ny, nz, cfg["nu"], cfg["Cs"], cfg["body_force"], cfg["Cd"],
+                        gpu.lad_from_spec(cfg["forest"], ny), flags, guard=1 << 16)
+            g.set_init(0, 0.05, 0.05)
+            if kind == "solid":
+                rng = np.random.default_rng(nx * 131 + ny)
+                g.set_solid((rng.random((nz, ny, nx)) < 0.15).astype(np.uint8))
+            g.init(7)
+            g.stats_accumulate(1)
+            if kind == "slab":
+                bufs = [g.halo_buffer() for _ in range(4)]
+                for _ in range(3):
+                    g.halo_pack(0, bufs[0]); g.halo_pack(1, bufs[1])
+                    g.halo_unpack(0, bufs[1]); g.halo_unpack(1, bufs[0])
+                    g.step(1)
+                    g.step_slab_begin(bufs[0], bufs[1], None)
+                    g.step_slab_end(bufs[1], bufs[0], None)
+            else:
+                g.set_graphs(0)
+                g.step(5)
+                g.set_graphs(1)
+                g.step(70)
+            if kind == "solid":
+                g.set_solid(None)
+                g.step(3)
+            g.get_macros(); g.stats_read(); st = g.get_state()
+            g.set_state(st, 3)
+            g.step(2)
+            rho = torch.empty(g.shape, dtype=torch.float32).pin_memory()
+            u = torch.empty((3,) + g.shape, dtype=torch.float32).pin_memory()
+            g.get_macros_host(rho, u)
+            g.set_macros_host(rho, u)
+            g.step(2)
+            assert g.guard_intact(), (nx, ny, nz, vec, bottom, top)
+            g.close()
+
+
+@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+def test_masked_update_is_run_to_run_bit_identical(gpu, aa):
+    """Five runs of a lattice with 15 % random solids (every lane takes the element-store path
+    somewhere) and of a plain one: identical to the last bit."""
+    import torch
+    for solid in (True, False):
+        cfg = wl.small(nx=96, ny=16, nz=12)
+        if solid:
+            rng = np.random.default_rng(5)
+            cfg["solid"] = (rng.random((12, 16, 96)) < 0.15).astype(np.uint8)
+        ref = None
+        for rep in range(5):
+            g = gpu.Lbm.from_config(cfg, aa=aa)
+            g.set_launch_shape(*[(24, 4), (8, 16), (12, 8), (24, 8), (6, 2)][rep]) if not solid else None
+            g.init(cfg["seed"])
+            g.stats_accumulate(1)
+            g.step(41)
+            st = g.get_state().cpu().numpy()
+            s, _ = g.stats_read()
+            g.close()
+            if ref is None:
+                ref = (st, s)
+            else:
+                assert np.array_equal(st, ref[0])
+                if solid:
+                    assert np.array_equal(s, ref[1])      # same block shape: same summation order
+                else:
+                    assert np.allclose(s, ref[1], rtol=0, atol=1e-9)
+
+
 def test_step_before_init_is_an_error(gpu):
     g = gpu.Lbm(8, 4, 4, 0.01, 0.1)
     with pytest.raises(gpu.LbmError) as e:
@@ -700,6 +794,105 @@ def test_p16_known_pi_neq_through_the_c_abi(orc, gpu, aa, t0):
         teeth = np.abs((1 / tau0 - 1 / tau_t) * fneq).max()
         assert err <= 3e-8 and teeth > 30 * 3e-8, (err, teeth)
         g.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# Row-table SGS models (lbm_set_sgs_rows, pin P19)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
+@pytest.mark.parametrize("t0", [0, 1])
+def test_p19_row_tables_through_the_c_abi(orc, gpu, aa, t0):
+    """Pin P19 on the CUDA path: a periodic uniform state with a known Pi_neq relaxes, row by row,
+    by (1 - 1/tau_j) with tau_j from the DEFINITION of the closure iterated to its fixed point
+    (damped constant, mean shear, clipped rows); then back to the standard model."""
+    import torch
+    c, w, _, _ = orc.tables()
+    c = c.astype(float)
+    rng = np.random.default_rng(191)
+    nx, ny, nz = 32, 6, 3
+    flags = gpu.bc_flags("periodic", "periodic", aa=aa)
+    B = rng.normal(size=(3, 3))
+    A = 0.5 * (B + B.T)
+    A -= np.trace(A) / 3 * np.eye(3)
+    A *= 3e-3 / np.sqrt(np.sum(A * A))
+    rho, u, nu, Cs = 1.04, np.array([0.08, -0.03, 0.02]), 3e-4, 0.17
+    tau0 = 3 * nu + 0.5
+    Qh = np.sqrt(np.sum(A * A))
+    S_now = 3.0 * Qh / (np.sqrt(2.0) * rho * tau0)
+    C_row = Cs ** 2 * np.array([0.0, 0.25, 1.0, 1.0, 2.0, 0.6])
+    S_row = S_now * np.array([0.0, 0.0, 0.5, 3.0, 0.9, 0.2])
+    cu = c @ u
+    feq = w * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u @ u))
+    fneq = w * 4.5 * np.einsum("iab,ab->i", np.einsum("ia,ib->iab", c, c) - np.eye(3) / 3, A)
+
+    def tau_def(Cj, Sj):
+        tau = tau0
+        for _ in range(200):
+            tau = tau0 + 3.0 * Cj * max(3.0 * Qh / (np.sqrt(2.0) * rho * tau) - Sj, 0.0)
+        return tau
+
+    g = gpu.Lbm(nx, ny, nz, nu, Cs, flags=flags)
+    st = torch.from_numpy(np.broadcast_to((feq + fneq - w)[:, None, None, None], (19, nz, ny, nx))
+                          .astype(np.float32).copy()).cuda()
+    for tables in ((C_row, S_row), (C_row, None), (None, S_row), (None, None)):
+        g.set_sgs_rows(*tables)
+        g.set_state(st, t0)
+        g.step(1)
+        got = g.get_state().double().cpu().numpy()
+        taus = []
+        for j in range(ny):
+            tau_j = tau_def(Cs ** 2 if tables[0] is None else C_row[j], 0.0 if tables[1] is None else S_row[j])
+            taus.append(tau_j)
+            want = feq + (1 - 1 / tau_j) * fneq - w
+            assert np.abs(got[:, :, j, :] - want[:, None, None]).max() <= 3e-8, (tables, j)
+        if tables[0] is not None and tables[1] is not None:
+            assert taus[3] == tau0 and taus[0] == tau0 and taus[2] > taus[4] > tau0     # clipped / active rows
+            assert np.abs((1 / taus[2] - 1 / tau0) * fneq).max() > 20 * 3e-8           # the test has teeth
+    with pytest.raises(gpu.LbmError):
+        g.set_sgs_rows(-C_row, None)
+    g.close()
+
+
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
+@pytest.mark.parametrize("nx,vec", [(64, 4), (34, 2), (33, 1)])
+@pytest.mark.parametrize("model", ["damped", "shear_improved"])
+def test_sgs_row_models_parity(orc, gpu, aa, nx, vec, model):
+    """Wall-damped and shear-improved Smagorinsky on a forced forest half-channel: 20 steps with
+    statistics, populations and plane statistics against the oracle.  The shear-improved table is
+    built from each side's own statistics of the first 10 steps (helper against helper too)."""
+    import torch
+    cfg = wl.small(nx=nx, ny=12, nz=8, Cs=0.17)
+    o, g = _pair(orc, gpu, cfg, aa, vec)
+    w = _weights(orc)
+    o.stats_accumulate(1); g.stats_accumulate(1)
+    if model == "damped":
+        Co = orc.sgs_van_driest(12, 0.17, 0.004, cfg["nu"], 26.0)
+        Cg = gpu.sgs_van_driest(12, 0.17, 0.004, cfg["nu"], 26.0)
+        assert np.allclose(Co, Cg, rtol=1e-13, atol=0)
+        o.set_sgs_rows(Co, None); g.set_sgs_rows(Cg, None)
+        o.step(20); g.step(20)
+    else:
+        o.step(10); g.step(10)
+        so, _ = o.stats_read()
+        sg, _ = g.stats_read()
+        So, Sg = orc.sgs_mean_shear(so, top_wall=False), gpu.sgs_mean_shear(sg, top_wall=False)
+        assert np.abs(So - Sg).max() <= 1e-5 * cfg["u_bulk"] and So.max() > 1e-3
+        # scaled down so that the closure is active on some rows and clipped on others
+        o.set_sgs_rows(None, 0.02 * So); g.set_sgs_rows(None, 0.02 * So)
+        o.step(10); g.step(10)
+    assert _state_err(o, g, w) <= 2e-7
+    er, eu = _macro_err(o, g)
+    assert er <= TOL_REL * cfg["u_bulk"] and eu <= TOL_REL * cfg["u_bulk"]
+    so, n1 = o.stats_read()
+    sg, n2 = g.stats_read()
+    assert n1 == n2 == 20
+    assert np.abs(sg[:, :3] - so[:, :3]).max() <= TOL_REL * cfg["u_bulk"]
+    # the model really acted: the standard model gives a different state
+    o2, g2 = _pair(orc, gpu, cfg, aa, vec)
+    g2.step(20)
+    torch.cuda.synchronize()
+    assert float((g2.get_state() - g.get_state()).abs().max()) > 1e-6
+    g.close(); g2.close()
 
 
 def test_divergence_is_reported(gpu):

@@ -167,3 +167,26 @@ def test_normalisation_helpers_closed_forms(lb):
         lb.stats_normalise(st, 0.0)
     yp = lb.wall_units(4, 0.01, 2e-4)
     assert np.allclose(yp, (np.arange(4) + 0.5) * 50.0)
+
+
+def test_sgs_row_table_helpers_closed_forms(lb):
+    """Host helpers of the row-table SGS models (include/lbm.h lbm_sgs_van_driest,
+    lbm_sgs_mean_shear) against their closed forms, written out here independently of oracle/."""
+    ny, Cs, ut, nu, Ap = 40, 0.1, 2.5e-3, 2e-4, 26.0
+    yp = (np.arange(ny) + 0.5) * ut / nu
+    C1 = lb.sgs_van_driest(ny, Cs, ut, nu, Ap)
+    assert np.allclose(C1, Cs ** 2 * (1 - np.exp(-yp / Ap)) ** 2, rtol=1e-13, atol=0)
+    C2 = lb.sgs_van_driest(ny, Cs, ut, nu, Ap, both_walls=True)
+    assert np.allclose(C2, C2[::-1], rtol=1e-15) and np.array_equal(C2[: ny // 2], C1[: ny // 2])
+    with pytest.raises(lb.LbmError):
+        lb.sgs_van_driest(ny, Cs, ut, 0.0)
+    y = np.arange(ny) + 0.5
+    st = np.zeros((ny, lb.NSTAT))
+    st[:, 0] = 0.2 * (y / ny) * (1 - y / ny)
+    st[:, 2] = -0.5 * st[:, 0]
+    S = lb.sgs_mean_shear(st, top_wall=True)
+    want = np.abs(0.2 / ny * (1 - 2 * y / ny)) * np.sqrt(1.25)
+    assert np.allclose(S[1:-1], want[1:-1], rtol=1e-12, atol=1e-18)
+    assert np.isclose(S[0], 0.5 * (st[0, 0] + st[1, 0]) * np.sqrt(1.25), rtol=1e-13) and np.isclose(S[-1], S[0], rtol=1e-12)
+    S2 = lb.sgs_mean_shear(st, top_wall=False)
+    assert np.isclose(S2[-1], 0.5 * abs(st[-1, 0] - st[-2, 0]) * np.sqrt(1.25), rtol=1e-12)

@@ -49,8 +49,8 @@ CONFIGS = {
     # BASELINE.json:configs[1]; F = u_tau^2/H, H = 64, u_tau = 180 nu / H (Eq. 16)
     "cfg2": _cfg("cfg2", 256, 128, 128, 2e-4, 0.1, 4.9438e-9, 0.0, BOUNCE_BACK, BOUNCE_BACK,
                  None, INIT_PARABOLA, 0.050625, 0.10,
-                 u_bulk=0.050625, steps=2000, stats_every=1,
-                 note="plane channel, nominal Re_tau=180"),
+                 u_bulk=0.050625, steps=2000, storage="aax", stats_every=1,
+                 note="plane channel, nominal Re_tau=180, single-array AA pattern (x-balanced)"),
     # BASELINE.json:configs[2]
     "cfg3": _cfg("cfg3", 512, 128, 256, 1e-4, 0.1, 3.968e-7, 0.15, BOUNCE_BACK, FREE_SLIP,
                  dict(kind="lalic", h=16, LAI=2.0, eta_m=0.7), INIT_POWER_LAW, 0.08, 0.05,
