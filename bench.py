@@ -382,7 +382,8 @@ def run_b200(args, cfg):
 
 
 def run_sharded(args, cfg):
-    """--sharded: ONE lattice of nx x ny x (N nz) cut into N z slabs (two-lattice storage), one
+    """--sharded: ONE lattice of nx x ny x (N nz) cut into N z slabs (two-lattice storage unless
+    --storage says aa / aax), one
     halo exchange per step over torch.distributed, overlapped with the interior update
     (DESIGN.md "Multi-GPU").  Opt-in: north_star asks for one GPU, so the default --gpus N path
     stays N replicas; on this run's hardware the NCCL leg could only be exercised with N = 1
@@ -409,11 +410,11 @@ def run_sharded(args, cfg):
 
     g = dict(cfg)
     g["nz"] = cfg["nz"] * world
-    g["storage"] = "two_lattice"
+    g["storage"] = args.storage or "two_lattice"
     K, W = args.steps, args.warmup
     N = wl.n_cells(cfg)
     every = cfg.get("stats_every", 0)
-    s = slab.SlabLbm(g, rank, world, device=dev)
+    s = slab.SlabLbm(g, rank, world, device=dev, storage=g["storage"])
     s.init(cfg["seed"])
     s.stats_accumulate(every)
     s.step(W)

@@ -62,8 +62,8 @@ typedef enum lbm_status {
                                              forest codes (lbm_set_forest_codes)                            */
 #define LBM_STORAGE_AA        (1u << 6)   /* bit 6: 0 two-lattice pull, 1 single-array AA pattern     */
 #define LBM_Z_HALO            (1u << 7)   /* bit 7: z slab of a larger lattice: planes 0 and nz-1 are ghost
-                                             planes filled by the halo calls, planes 1..nz-2 are updated
-                                             (two-lattice storage only)                                     */
+                                             planes served by the halo calls, planes 1..nz-2 are updated
+                                             (any storage scheme)                                           */
 #define LBM_VEC_SHIFT         8           /* bits 8-10: cells per thread override (0 auto, 1, 2, 4)   */
 #define LBM_VEC_MASK          (7u << 8)
 #define LBM_STORAGE_AAX       (1u << 11)  /* bit 11: single array, x-balanced AA pattern: as LBM_STORAGE_AA in
@@ -167,10 +167,15 @@ int lbm_step(lbm_t *h, int n);
  * points is required").  The handle is created with nz = nz_local + 2.  After
  * lbm_init / lbm_set_macros* and after every lbm_step(1) the caller exchanges the two faces with
  * its z neighbours: lbm_halo_pack(side, buf) copies the five populations leaving through the low
- * (side 0: c_z = -1, plane 1) or high (side 1: c_z = +1, plane nz-2) face into the device buffer
- * [5][ny][nx] fp32; the neighbour passes the buffer it received to lbm_halo_unpack(side, buf),
- * side = the side of ITS OWN slab the data enters through (0: ghost plane 0 takes c_z = +1 data,
- * 1: ghost plane nz-1 takes c_z = -1 data).  All asynchronous on the bound stream.
+ * (side 0) or high (side 1) face into the device buffer [5][ny][nx] fp32; the neighbour passes the
+ * buffer it received to lbm_halo_unpack(side, buf), side = the side of ITS OWN slab the data enters
+ * through.  Where the five populations sit depends on the storage scheme and the time parity, and
+ * the library knows (two-lattice: c_z = -1 of plane 1 / c_z = +1 of plane nz-2 leave and land in
+ * the neighbour's ghost planes; single array at odd t: the same planes, opposite slot sets; single
+ * array at even t: what leaves has been pushed into the ghost planes and lands in the neighbour's
+ * boundary plane, except where the destination cell bounced its own population off a wall face or
+ * a solid cell).  The caller only has to keep all slabs of a lattice on the same storage scheme.
+ * All asynchronous on the bound stream.
  * lbm_set_z_slab tells the synthetic initial field where the slab sits: local plane 0 (the low
  * ghost) is global plane z_first - 1 of nz_global (periodic).  Statistics and lbm_get_macros
  * cover the interior planes (ghost-plane entries of lbm_get_macros are meaningless); plane
@@ -194,7 +199,7 @@ int lbm_halo_unpack(lbm_t *h, int side, const float *buf_dev);
  *                        into recv_hi, and records ready_event there: the transfer runs while the
  *                        interior planes are being updated.
  *   lbm_step_slab_end    makes the bound stream wait for ready_event (NULL = no wait), unpacks the
- *                        two buffers into the ghost planes of the new state, runs the statistics
+ *                        two buffers into the new state (ghost or boundary planes), runs the statistics
  *                        stage 2 of a sampled step and advances lbm_time.  Asynchronous.
  * Results are bit-identical to the sequential form.  LBM_ESTATE if the calls do not alternate;
  * LBM_EINVAL without LBM_Z_HALO. */

@@ -61,7 +61,10 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     size_t off = 0;
     L.pops = off; off = align_up(off + (size_t)Q * N * 4, 256);
     L.pops2 = off; if (!aa) off = align_up(off + (size_t)Q * N * 4, 256);
-    const int pmax = (nx / TMA_BOX > MAX_NCHUNK) ? nx / TMA_BOX : MAX_NCHUNK;
+    // partials per row: x chunks of the step launch (<= MAX_NCHUNK), TMA tiles, or - geometry handles - one
+    // per warp of a row (KParams::wpart)
+    int pmax = (nx / TMA_BOX > MAX_NCHUNK) ? nx / TMA_BOX : MAX_NCHUNK;
+    if (mask && (nx + 31) / 32 > pmax) pmax = (nx + 31) / 32;
     L.partial = off; off = align_up(off + (size_t)ny * NSTAT * nz * pmax * 4, 256);
     L.acc = off; off = align_up(off + (size_t)ny * NSTAT * 8, 256);
     L.shift = off; off = align_up(off + (size_t)ny * 4 * 4, 256);
@@ -97,6 +100,7 @@ struct lbm_s {
     bool partial_launches;      // some launches cover only part of the planes (TY must divide ny)
     bool forest_codes;          // per-cell forest codes installed (geometry handles)
     bool sgs_rows;              // per-row SGS table installed (lbm_set_sgs_rows)
+    long long nflagged;         // thread blocks of the step launch that hold geometry (rebuild_block_flags)
     bool slab_open, slab_sample; // between lbm_step_slab_begin and _end; that step samples
     int zg0, nzg;               // z slab: global plane of local plane 0, global nz
     int zlo, zhi;               // planes the step updates: [zlo, zhi)
@@ -167,10 +171,18 @@ static void set_variant(lbm_s *h)
 // The statistics partials are laid out with `pchunks` x chunks per row: the larger of the
 // chunkings of the kernels in use.  When it changes the buffer is cleared (entries no kernel
 // writes must read as zero in the stage-2 sum).
-static int set_pchunks(lbm_s *h)
+static bool warp_partials(const lbm_s *h) { return h->mask && (h->TX % 32) == 0; }   // KParams::wpart
+static int want_pchunks(const lbm_s *h)
 {
     int pc = h->nchunk;
     if (h->tma_mode && h->nx / TMA_BOX > pc) pc = h->nx / TMA_BOX;
+    if (warp_partials(h)) pc = h->nchunk * (h->TX / 32);
+    return pc;
+}
+static int set_pchunks(lbm_s *h)
+{
+    const int pc = want_pchunks(h);
+    h->kp.wpart = warp_partials(h) ? 1 : 0;
     if (pc != h->pchunks) {
         h->pchunks = pc;
         graph_drop(h);
@@ -260,7 +272,6 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     if ((bc_flags & LBM_STORAGE_AAX) && (bc_flags & LBM_SOLID_MASK))
         return fail(LBM_EINVAL, "LBM_STORAGE_AAX has no geometry variant: use LBM_STORAGE_AA or two-lattice storage with LBM_SOLID_MASK");
     if (bc_flags & LBM_Z_HALO) {
-        if (bc_flags & (LBM_STORAGE_AA | LBM_STORAGE_AAX)) return fail(LBM_EINVAL, "LBM_Z_HALO needs two-lattice storage");
         if (nz < 3) return fail(LBM_EINVAL, "LBM_Z_HALO needs nz >= 3 (two ghost planes + >= 1 interior)");
     }
     const int V = pick_vec(nx, bc_flags);
@@ -309,8 +320,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
             if (got >= 2 && (r == 1 || r == 2 || r == 4) && ny % r == 0) h->tma_rows = r;
         }
     }
-    h->pchunks = h->nchunk;
-    if (h->tma_mode && nx / TMA_BOX > h->pchunks) h->pchunks = nx / TMA_BOX;
+    h->pchunks = want_pchunks(h);
     h->sweep = 1;
     {
         const char *e = getenv("LBM_SWEEP");        // A-B override: 0 = always forward
@@ -328,6 +338,7 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
     h->Utop[0] = h->Utop[1] = h->Utop[2] = 0.0;
     h->forest_codes = false;
     h->sgs_rows = false;
+    h->nflagged = 0;
     h->slab_open = false; h->slab_sample = false;
     set_variant(h);
     *out = h;
@@ -361,6 +372,7 @@ static void fill_params(lbm_s *h)
     p.src = reinterpret_cast<float *>(h->ws + h->L.pops);
     p.dst = h->aa ? p.src : reinterpret_cast<float *>(h->ws + h->L.pops2);
     p.nx = h->nx; p.ny = h->ny; p.nz = h->nz; p.nchunk = h->nchunk; p.pchunks = h->pchunks; p.N = h->N;
+    p.wpart = warp_partials(h) ? 1 : 0;
     const double tau0 = 3.0 * h->nu + 0.5;              // R3
     p.tau0 = (float)tau0; p.tau0sq = (float)(tau0 * tau0);
     p.ksmag = (float)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs); // R9: C_smag = Cs^2
@@ -459,6 +471,7 @@ int lbm_bind(lbm_t *h, void *dev_workspace, size_t bytes, void *cuda_stream)
         CU_TRY(cudaMemsetAsync(h->ws + h->L.solid, 0, mbytes, h->stream));
         CU_TRY(cudaMemsetAsync(h->ws + h->L.solid_nb, 0, mbytes, h->stream));
         CU_TRY(cudaMemsetAsync(h->ws + h->L.bflag, 0, (size_t)h->ny * h->nz * MAX_NCHUNK, h->stream));
+        h->nflagged = 0;
         h->forest_codes = false;
         h->kp.fidx = nullptr;
     }
@@ -477,6 +490,15 @@ static int rebuild_block_flags(lbm_s *h)
         h->kp, h->TX * h->V, h->TY, reinterpret_cast<unsigned char *>(h->ws + h->L.bflag), nblocks);
     h->launches++;
     CU_TRY(cudaGetLastError());
+    // how many blocks hold geometry: none (a mask that is all fluid, e.g. after the trip boxes have
+    // been removed) => lbm_step launches the plain kernels, at no cost at all
+    std::vector<unsigned char> flags((size_t)nblocks);
+    CU_TRY(cudaMemcpyAsync(flags.data(), h->ws + h->L.bflag, (size_t)nblocks, cudaMemcpyDeviceToHost, h->stream));
+    CU_TRY(cudaStreamSynchronize(h->stream));
+    long long n = 0;
+    for (unsigned char f : flags) n += f ? 1 : 0;
+    h->nflagged = n;
+    graph_drop(h);
     return LBM_OK;
 }
 
@@ -486,6 +508,9 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
     DevGuard dg(h);
     if (!h->mask) return fail(LBM_EINVAL, "handle was not created with LBM_SOLID_MASK");
     if (!h->bound) return fail(LBM_ESTATE, "lbm_set_solid before lbm_bind");
+    if (h->inited && h->halo && h->aa && (h->t & 1) == 0)
+        return fail(LBM_ESTATE, "on a single-array z slab a running mask change needs an odd time step "
+                                "(at even t populations of the neighbour slabs sit in this slab's planes)");
     const int nxw = (h->nx + 31) / 32;
     const size_t words = (size_t)nxw * h->ny * h->nz;
     std::vector<uint32_t> bits;
@@ -707,7 +732,8 @@ static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
 {
     StepLaunch L;
     L.TX = h->TX; L.TY = h->TY; L.nchunk = h->nchunk; L.nx = h->nx; L.ny = h->ny;
-    L.mask = h->mask; L.aa = h->aa; L.aax = h->aax; L.odd = (h->t & 1) != 0;
+    L.mask = h->mask && h->nflagged > 0;      // nothing flagged: the plain kernels
+    L.aa = h->aa; L.aax = h->aax; L.odd = (h->t & 1) != 0;
     L.tma_mode = h->tma_mode; L.tma_rows = h->tma_rows;
     // the map of the array this step reads (two-lattice: the roles swap every step)
     const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
@@ -1024,6 +1050,35 @@ int lbm_halo_bytes(const lbm_t *h, size_t *bytes)
     return LBM_OK;
 }
 
+// Which plane and which slot set (1: c_z = +1, 0: c_z = -1) a face of a slab in state t moves.
+//   two-lattice        : populations leave from the boundary planes and enter the ghost planes;
+//   single array, t odd : every population sits in the opposite slot of its own cell - the same
+//                        planes, the opposite slot sets;
+//   single array, t even: population i of cell x sits at slot i of cell x + c_i - what leaves has
+//                        been pushed into the ghost planes and enters the neighbour's boundary plane
+//                        (filtered: halo_kernel).
+struct HaloMap { int z, slots; bool filter; };
+static HaloMap halo_map(const lbm_s *h, long long t, int face, bool pack)
+{
+    const int nz = h->nz;
+    if (!h->aa) return pack ? HaloMap{face ? nz - 2 : 1, face, false} : HaloMap{face ? nz - 1 : 0, face ? 0 : 1, false};
+    if (t & 1) return pack ? HaloMap{face ? nz - 2 : 1, face ? 0 : 1, false} : HaloMap{face ? nz - 1 : 0, face, false};
+    return pack ? HaloMap{face ? nz - 1 : 0, face, false} : HaloMap{face ? nz - 2 : 1, face ? 0 : 1, true};
+}
+
+// pack / unpack one face of the array `arr` holding state t
+static cudaError_t halo_launch(lbm_s *h, float *arr, long long t, int face, float *buf, bool pack)
+{
+    const HaloMap m = halo_map(h, t, face, pack);
+    const long long plane = (long long)h->nx * h->ny;
+    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
+    if (pack) halo_kernel<true, false><<<blocks, 256, 0, h->stream>>>(h->kp, arr, m.z, m.slots, buf);
+    else if (m.filter) halo_kernel<false, true><<<blocks, 256, 0, h->stream>>>(h->kp, arr, m.z, m.slots, buf);
+    else halo_kernel<false, false><<<blocks, 256, 0, h->stream>>>(h->kp, arr, m.z, m.slots, buf);
+    h->launches++;
+    return cudaGetLastError();
+}
+
 static int halo_copy(lbm_s *h, int side, float *buf, bool pack)
 {
     if (!h) return fail(LBM_EINVAL, "handle is NULL");
@@ -1032,19 +1087,8 @@ static int halo_copy(lbm_s *h, int side, float *buf, bool pack)
     if (!h->inited) return fail(LBM_ESTATE, "halo call before lbm_init / lbm_set_macros");
     if (!buf || (side != 0 && side != 1)) return fail(LBM_EINVAL, "bad halo arguments");
     KParams p = h->kp;
-    if (h->t & 1) { float *t = p.src; p.src = p.dst; p.dst = t; }   // the lattice holding state t
-    const long long plane = (long long)h->nx * h->ny;
-    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
-    if (pack) {
-        // leaving data: low face = c_z -1 populations of plane 1, high face = c_z +1 of plane nz-2
-        halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.src, h->N, plane, side ? h->nz - 2 : 1, side, buf);
-    } else {
-        // entering data: through the low face (ghost plane 0) come c_z +1 populations, through the
-        // high face (ghost plane nz-1) c_z -1 populations
-        halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.src, h->N, plane, side ? h->nz - 1 : 0, side ? 0 : 1, buf);
-    }
-    h->launches++;
-    CU_TRY(cudaGetLastError());
+    if (!h->aa && (h->t & 1)) { float *t = p.src; p.src = p.dst; p.dst = t; }   // the lattice holding state t
+    CU_TRY(halo_launch(h, p.src, h->t, side, buf, pack));
     return LBM_OK;
 }
 
@@ -1078,12 +1122,8 @@ int lbm_step_slab_begin(lbm_t *h, float *send_lo_dev, float *send_hi_dev, void *
         p.z0 = zh - 1; p.z1 = zh;
         if ((rc = launch_step_timed(h, p, sample))) return rc;
     }
-    const long long plane = (long long)h->nx * h->ny;
-    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
-    halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, 1, 0, send_lo_dev);
-    halo_kernel<true><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, h->nz - 2, 1, send_hi_dev);
-    h->launches += 2;
-    CU_TRY(cudaGetLastError());
+    CU_TRY(halo_launch(h, p.dst, h->t + 1, 0, send_lo_dev, true));      // p.dst holds state t+1
+    CU_TRY(halo_launch(h, p.dst, h->t + 1, 1, send_hi_dev, true));
     if (packed_event) CU_TRY(cudaEventRecord(static_cast<cudaEvent_t>(packed_event), h->stream));
     if (zh - 1 > zl + 1) {
         p.z0 = zl + 1; p.z1 = zh - 1;
@@ -1102,14 +1142,9 @@ int lbm_step_slab_end(lbm_t *h, const float *recv_lo_dev, const float *recv_hi_d
     if (!recv_lo_dev || !recv_hi_dev) return fail(LBM_EINVAL, "receive buffer is NULL");
     if (ready_event) CU_TRY(cudaStreamWaitEvent(h->stream, static_cast<cudaEvent_t>(ready_event), 0));
     const KParams p = step_params(h, false);              // p.dst holds state t+1
-    const long long plane = (long long)h->nx * h->ny;
-    const unsigned blocks = (unsigned)((5 * plane + 255) / 256);
-    // through the low face (ghost plane 0) come the c_z = +1 populations, through the high face
-    // (ghost plane nz-1) the c_z = -1 ones
-    halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, 0, 1, const_cast<float *>(recv_lo_dev));
-    halo_kernel<false><<<blocks, 256, 0, h->stream>>>(p.dst, h->N, plane, h->nz - 1, 0, const_cast<float *>(recv_hi_dev));
-    h->launches += 2;
-    CU_TRY(cudaGetLastError());
+    // what entered through the low face comes from the lower neighbour's high face and vice versa
+    CU_TRY(halo_launch(h, p.dst, h->t + 1, 0, const_cast<float *>(recv_lo_dev), false));
+    CU_TRY(halo_launch(h, p.dst, h->t + 1, 1, const_cast<float *>(recv_hi_dev), false));
     if (h->slab_sample) {
         CU_TRY(launch_stage2(h, 0));
         h->nsamples++;

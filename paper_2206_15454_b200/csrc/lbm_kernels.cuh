@@ -76,6 +76,9 @@ struct KParams {
     int nx, ny, nz;
     int nchunk;          // blocks per x row
     int pchunks;         // x chunks per row in the layout of `partial` (>= nchunk of any kernel in use)
+    int wpart;           // 1 = every warp of a row segment stores its own partial (no block-level reduce;
+                         //     pchunks = nchunk * warps per segment): geometry handles, where one warp of a
+                         //     block may take the slow geometry path and the others should not wait for it
     long long N;
     // physics (fp32 copies)
     float tau0, tau0sq, ksmag;  // ksmag = 18 sqrt(2) Cs^2
@@ -395,6 +398,18 @@ __device__ __forceinline__ unsigned solid_nb_word(const KParams &p, const Ctx &c
 }
 
 template <int V>
+__device__ __forceinline__ unsigned long long solid_gather_rows(const KParams &p, const Ctx &c)
+{
+    const int ys[3] = {c.ym, c.y, c.yp}, zs[3] = {c.zm, c.z, c.zp};
+    unsigned long long S = 0ull;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+            S |= (unsigned long long)solid_field<V>(p, c, ys[a], zs[b]) << (6 * (3 * a + b));
+    return S;
+}
+template <int V>
 __device__ __forceinline__ unsigned long long solid_gather(const KParams &p, const Ctx &c, unsigned nb)
 {
     // if no cell within one step is solid every field is zero and the nine-row gather is skipped
@@ -469,22 +484,37 @@ __device__ __forceinline__ void solid_fix_loads(const KParams &p, const Ctx &c, 
 {
     if constexpr (RM == RD_LOCAL) return;
     static_assert(RM == RD_LOCAL || RM == RD_PULL || RM == RD_PULL_OPP, "the geometry variants exist for two-lattice and AA storage");
-    static_for<1, Q>([&](auto ic) {
+    // Which cells of direction i bounce: the bits of the source cells x0+k - c_x in the row load_dir used.
+    auto bounce_bits = [&](auto ic) -> unsigned {
         constexpr int i = decltype(ic)::value;
         constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
         bool bb = false, fs = false;
         if constexpr (cy == 1) bb = c.bot_bb;
         if constexpr (cy == -1) { bb = c.top_bb; fs = c.top_fs; }
         const int a = (bb || fs) ? 1 : 1 - cy, b = bb ? 1 : 1 - cz;
-        const unsigned bits = bb ? 0u : (solid_pick(S, a, b) >> (1 - cx)) & ((1u << V) - 1u);
-        if (bits) {
+        return bb ? 0u : (solid_pick(S, a, b) >> (1 - cx)) & ((1u << V) - 1u);
+    };
+    // The own-cell loads of the bouncing links are issued in batches of six directions and consumed
+    // afterwards: three dependent round trips to memory instead of up to eighteen.
+    const float *ownp = p.src + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0);
+    static_for<0, 3>([&](auto bc) {
+        constexpr int i0 = 1 + 6 * decltype(bc)::value;
+        float own[6][V];
+        unsigned bits[6];
+        static_for<0, 6>([&](auto jc) {
+            constexpr int j = decltype(jc)::value, i = i0 + j;
             constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[i] : i;
-            float own[V];
-            ldv<V>(p.src + (long long)S_BB * p.N + ((long long)(c.y + p.ny * c.z) * p.nx + c.x0), own);
+            bits[j] = bounce_bits(std::integral_constant<int, i>{});
+            if (bits[j]) ldv<V>(ownp + (long long)S_BB * p.N, own[j]);
+        });
+        static_for<0, 6>([&](auto jc) {
+            constexpr int j = decltype(jc)::value, i = i0 + j;
+            if (bits[j]) {
 #pragma unroll
-            for (int k = 0; k < V; ++k)
-                if ((bits >> k) & 1u) g[i][k] = own[k];
-        }
+                for (int k = 0; k < V; ++k)
+                    if ((bits[j] >> k) & 1u) g[i][k] = own[j][k];
+            }
+        });
     });
 }
 
@@ -807,6 +837,8 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
         const int wpr = TX >> 5;
         if (wpr == 1) {
             if (owner) out[(long long)col * pstride] = v4;
+        } else if (p.wpart) {
+            if (owner) out[(long long)col * pstride + (long long)c.chunk * (wpr - 1) + (tx >> 5)] = v4;
         } else {
             if (owner) sred[warp][col] = v4;
             __syncthreads();
@@ -827,14 +859,39 @@ __device__ __forceinline__ void stats_row_reduce(const KParams &p, const Ctx &c,
             for (int k = 0; k < NSTAT; ++k) out[(long long)k * pstride] = s[k];
         }
     } else {
-        // irregular width: go through shared memory
+        // irregular width (the paper's 350- and 372-cell meshes: 175, 93 threads per row): through
+        // shared memory; every FULL warp of the block then reduces whole row segments - each lane sums
+        // the entries lane, lane + 32, ... of the ten columns, the butterfly finishes - and the
+        // owner lanes store.  Blocks smaller than a warp sum serially.
+        const int TY = blockDim.y;
 #pragma unroll
         for (int k = 0; k < NSTAT; ++k) srow[lin][k] = s[k];
         __syncthreads();
-        for (int k = tx; k < NSTAT; k += TX) {   // TX may be smaller than NSTAT
-            float v = 0.f;
-            for (int q = 0; q < TX; ++q) v += srow[ty * TX + q][k];
-            out[(long long)k * pstride] = v;
+        const int nfull = (TX * TY) >> 5;
+        if (nfull == 0) {
+            for (int k = tx; k < NSTAT; k += TX) {   // TX may be smaller than NSTAT
+                float v = 0.f;
+                for (int q = 0; q < TX; ++q) v += srow[ty * TX + q][k];
+                out[(long long)k * pstride] = v;
+            }
+        } else if (warp < nfull) {
+            const int row0 = c.z * p.ny + c.y - ty;          // row of segment 0 of this block
+            for (int seg = warp; seg < TY; seg += nfull) {
+                float v[NSTAT];
+#pragma unroll
+                for (int k = 0; k < NSTAT; ++k) v[k] = 0.f;
+                for (int q = lane; q < TX; q += 32) {
+#pragma unroll
+                    for (int k = 0; k < NSTAT; ++k) v[k] += srow[seg * TX + q][k];
+                }
+                float v4;
+                bool owner;
+                int col;
+                stats_warp_butterfly(v, lane, v4, owner, col);
+                const int row = row0 + seg, z = row / p.ny, y = row - z * p.ny;
+                if (owner)
+                    p.partial[((long long)y * NSTAT + col) * pstride + (long long)z * p.pchunks + c.chunk] = v4;
+            }
         }
     }
 }
@@ -856,19 +913,17 @@ template <int V, int RM, int WM, bool STATS, bool MASK, bool SGS>
 __device__ __forceinline__ void step_body(const KParams &p)
 {
     const Ctx c = make_ctx<V>(p, p.z0 * p.ny);
-    // With a mask, a warp none of whose lanes has a solid cell within one step (the usual case:
-    // geometry is sparse) runs the unmasked load/store code; the decision is warp-uniform, so the
-    // full-mask shuffles inside load_dir/store_dir stay converged.
-    // (the mask word is requested first and looked at only after the 19 population loads have
-    // been issued, so it adds no latency to them)
-    unsigned nbw = 0u;
-    if constexpr (MASK) nbw = solid_nb_word(p, c);
+    // Geometry body (only blocks flagged by blockflag_kernel come here): the nine-row gather of the
+    // solid bits is requested BEFORE the 19 population loads, so both travel together and the only
+    // dependent round trip left is the own-cell loads of the links that bounce.  A warp none of
+    // whose lanes has a solid cell within one step runs the unmasked load/store code; the decision
+    // is warp-uniform, so the full-mask shuffles inside load_dir/store_dir stay converged.
+    unsigned long long S = 0ull;
+    if constexpr (MASK) S = solid_gather_rows<V>(p, c);
     float g[Q][V];
     load_all<V, RM>(p, c, g);
-    unsigned long long S = 0ull;
     bool geom = false;
     if constexpr (MASK) {
-        S = solid_gather<V>(p, c, nbw);
         geom = __any_sync(0xffffffffu, S != 0ull);
         if (geom) solid_fix_loads<V, RM>(p, c, g, S);
     }
@@ -911,6 +966,9 @@ __device__ __forceinline__ void step_body(const KParams &p)
 template <int V, int RM, int WM, bool STATS, bool MASK = false, bool SGS = false>
 __global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
 {
+    // (The geometry body as a __noinline__ function of its own, so that the plain body keeps the
+    // register allocation of the kernel without MASK, was measured: slower - cfg3 boxes + statistics
+    // 39.2 against 39.7 GLUPS, cfg4 all-fluid mask -4.7 % against -0.7 % - and dropped.)
     if constexpr (MASK) {
         const long long gb = (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
         if (__ldg(p.bflag + gb) == 0) {
@@ -1228,19 +1286,45 @@ static __global__ void __launch_bounds__(256) stats_stage2_kernel(const float *_
 
 // ---------------------------------------------------------------------------------------------
 // z-slab halo exchange: the five populations that cross a z face, of one x-y
-// plane, to / from a contiguous buffer [5][ny][nx].  side 1: c_z = +1 (i = 5, 11, 14, 15, 18),
-// side 0: c_z = -1 (i = 6, 12, 13, 16, 17).  pack reads plane `z`, unpack writes plane `z`.
+// plane, to / from a contiguous buffer [5][ny][nx].  side 1: slots with c_z = +1 (i = 5, 11, 14, 15,
+// 18), side 0: slots with c_z = -1 (i = 6, 12, 13, 16, 17).  pack reads plane `z`, unpack writes
+// plane `z`.  Which plane and which slot set a face exchange moves depends on the storage scheme
+// and the time parity (lbm_api.cu: halo_map).
+//
+// FILTER (unpack only): the single-array storages at even t keep population i of cell x at slot i
+// of cell x + c_i ("push" representation), so what crosses the face is the neighbour rank's ghost
+// plane, going into the slots of REAL cells of the boundary plane.  Only entries that a cell of the
+// ghost plane has written may land: an entry whose source cell lies beyond a wall / lid face or is
+// solid holds the destination cell's own bounced population and stays; nothing lands in a solid cell.
 // ---------------------------------------------------------------------------------------------
-template <bool PACK>
-__global__ void halo_kernel(float *pops, long long N, long long plane, int z, int side, float *buf)
+template <bool PACK, bool FILTER>
+__global__ void halo_kernel(const KParams p, float *pops, int z, int side, float *buf)
 {
+    const long long plane = (long long)p.nx * p.ny;
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= 5 * plane) return;
     const int j = (int)(q / plane);
     const long long r = q - (long long)j * plane;
     const int up[5] = {5, 11, 14, 15, 18}, dn[5] = {6, 12, 13, 16, 17};
     const int i = side ? up[j] : dn[j];
-    float *cell = pops + (long long)i * N + (long long)z * plane + r;
+    if constexpr (FILTER) {
+        const int cxs[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+        const int cys[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+        const int y = (int)(r / p.nx), x = (int)(r - (long long)y * p.nx);
+        int ys = y - cys[i];
+        if (ys < 0) {
+            if (p.bot == BC_BOT_PERIODIC) ys = p.ny - 1; else return;       // the cell's own bounce off the wall
+        } else if (ys >= p.ny) {
+            if (p.top == BC_TOP_PERIODIC) ys = 0;
+            else if (p.top == BC_TOP_SLIP) ys = y;                          // mirrored link from the same row
+            else return;
+        }
+        int xs = x - cxs[i];
+        xs = (xs < 0) ? p.nx - 1 : (xs >= p.nx ? 0 : xs);
+        const int zs = side ? z - 1 : z + 1;                                 // the ghost plane it came from
+        if (p.solid && (solid_at(p, x, y, z) || solid_at(p, xs, ys, zs))) return;
+    }
+    float *cell = pops + (long long)i * p.N + (long long)z * plane + r;
     if (PACK) buf[q] = *cell; else *cell = buf[q];
 }
 

@@ -12,10 +12,12 @@ CUDA stream that waits for that event while the library's stream updates the int
 the unpack waits for the exchange (lbm.h: lbm_step_slab_begin / _end).
 
 Rank r of W owns the global planes [r nz/W, (r+1) nz/W) plus one ghost plane on either side; z is
-periodic, so the ranks form a ring.  The slab uses the two-lattice storage (the in-place AA
-pattern would push into the ghost planes).  north_star runs on one GPU: this is the path the
-lattice would take beyond one GPU's 180 GB, verified by emulating the ranks one after another on
-one GPU (bit-identical to the undivided lattice) and by gloo ring tests on the CPU.
+periodic, so the ranks form a ring.  Any storage scheme: two-lattice (default), or the single-array
+AA / x-balanced AA patterns at half the memory (the in-place odd step pushes into the ghost planes;
+the library moves those planes to the neighbour's boundary plane instead - the calls are the
+same).  north_star runs on one GPU: this is the path the lattice would take beyond one GPU's
+180 GB, verified by emulating the ranks one after another on one GPU (bit-identical to the
+undivided lattice) and by gloo ring tests on the CPU.
 """
 from __future__ import annotations
 
@@ -54,7 +56,7 @@ class SlabLbm:
     torch.distributed's default group (world == 1: the slab is its own neighbour)."""
 
     def __init__(self, cfg: dict, rank: int = 0, world: int = 1, device="cuda:0", group=None,
-                 emulated: bool = False):
+                 emulated: bool = False, storage: str = "two_lattice"):
         if cfg["nz"] % world:
             raise ValueError(f"nz={cfg['nz']} is not a multiple of the number of slabs {world}")
         self.rank, self.world, self.group = int(rank), int(world), group
@@ -67,7 +69,10 @@ class SlabLbm:
         if cfg.get("solid") is not None:                        # local planes incl. the two ghosts
             z = np.arange(self.z_first - 1, self.z_first + self.nz_local + 1) % self.nz_global
             local["solid"] = np.asarray(cfg["solid"])[z]
-        self.sim = Lbm.from_config(local, aa=False, halo=True, device=device)
+        if storage not in ("two_lattice", "aa", "aax"):
+            raise ValueError(f"unknown storage scheme {storage!r}")
+        aa = {"two_lattice": False, "aa": True, "aax": "aax"}[storage]
+        self.sim = Lbm.from_config(local, aa=aa, halo=True, device=device)
         self.sim.set_z_slab(self.z_first, self.nz_global)
         self.cfg = cfg
         self._send = [self.sim.halo_buffer(), self.sim.halo_buffer()]    # [lo, hi]

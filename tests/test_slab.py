@@ -78,30 +78,38 @@ def test_ring_exchange_single_rank_is_self_periodic():
 # GPU: emulated ring == undivided lattice
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.gpu
+@pytest.mark.parametrize("storage", ["two_lattice", "aa", "aax"])
 @pytest.mark.parametrize("world", [1, 2, 3, 4])
-@pytest.mark.parametrize("case", ["forest", "lid+solid"])
-def test_emulated_slabs_equal_global_lattice(world, case):
+@pytest.mark.parametrize("case", ["forest", "lid+solid", "slip+solid", "periodic"])
+def test_emulated_slabs_equal_global_lattice(world, case, storage):
     import torch
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2206_15454_b200 as lb
     from paper_2206_15454_b200 import slab
 
+    if storage == "aax" and "solid" in case:
+        pytest.skip("the x-balanced AA storage has no geometry variant")
     cfg = wl.small(nx=32, ny=10, nz=12)
-    if case == "lid+solid":
-        cfg = wl.small(nx=32, ny=10, nz=12, top=wl.FORCED_EQ)
-        cfg["U_top"] = (0.06, 0.0, 0.01)
+    if case == "periodic":
+        cfg = wl.small(nx=32, ny=10, nz=12, bottom=wl.PERIODIC, top=wl.PERIODIC)
+    if "solid" in case:
+        if case == "lid+solid":
+            cfg = wl.small(nx=32, ny=10, nz=12, top=wl.FORCED_EQ)
+            cfg["U_top"] = (0.06, 0.0, 0.01)
         m = np.zeros((12, 10, 32), bool)
         m[0:2, 0:3, 4:9] = True                          # a box that straddles the z wrap ...
         m[11, 0:3, 4:9] = True
         m[5:7, 2:5, 30:] = True                          # ... and one across a slab face and the x wrap
         m[5:7, 2:5, :2] = True
+        m[2:4, 7:10, 12:15] = True                       # ... and one under the top face, across a slab face
         cfg["solid"] = m
-    ref = lb.Lbm.from_config(cfg, aa=False)
+    aa = {"two_lattice": False, "aa": True, "aax": "aax"}[storage]
+    ref = lb.Lbm.from_config(cfg, aa=aa)
     ref.init(cfg["seed"])
     ref.stats_accumulate(1)
     ref.stats_reset()
-    slabs = [slab.SlabLbm(cfg, r, world, emulated=True) for r in range(world)]
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True, storage=storage) for r in range(world)]
     slab.init_emulated(slabs, cfg["seed"])
     for s in slabs:
         s.stats_accumulate(1)
@@ -112,7 +120,7 @@ def test_emulated_slabs_equal_global_lattice(world, case):
         rr, ur = ref.get_macros()
         rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
         us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
-        if case == "forest":
+        if "solid" not in case:
             assert torch.equal(rs, rr) and torch.equal(us, ur), (world, n)
         else:
             # geometry handles run the plain or the geometry body per thread block (two
@@ -159,8 +167,6 @@ def test_halo_flag_rules():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2206_15454_b200 as lb
-    with pytest.raises(lb.LbmError):                      # AA storage pushes into the ghost planes
-        lb.Lbm(32, 4, 6, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip", aa=True, halo=True))
     with pytest.raises(lb.LbmError):
         lb.Lbm(32, 4, 2, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip", halo=True))
     g = lb.Lbm(32, 4, 6, 0.01, 0.1, flags=lb.bc_flags("bounce_back", "free_slip"))
@@ -169,8 +175,9 @@ def test_halo_flag_rules():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("storage", ["two_lattice", "aa"])
 @pytest.mark.parametrize("world", [1, 2, 3])
-def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
+def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world, storage):
     """The begin / exchange-on-a-second-stream / end form (lbm_step_slab_begin/_end): re-assembled
     slab fields against the ORACLE over 20 steps at the north_star tolerance, and to a few ulp
     against the undivided CUDA lattice (a geometry handle: see the note in the test above; without
@@ -187,9 +194,9 @@ def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
     cfg["solid"] = m
     o = orc.Oracle.from_config(cfg)
     o.init_from_config(cfg)
-    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref = lb.Lbm.from_config(cfg, aa=(storage == "aa"))
     ref.init(cfg["seed"])
-    slabs = [slab.SlabLbm(cfg, r, world, emulated=True) for r in range(world)]
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True, storage=storage) for r in range(world)]
     slab.init_emulated(slabs, cfg["seed"])
     for s in slabs:
         s.stats_accumulate(1)
@@ -223,7 +230,8 @@ def test_overlapped_slabs_equal_the_lattice_and_the_oracle(orc, world):
 
 
 @pytest.mark.gpu
-def test_single_slab_overlapped_through_the_comm_stream():
+@pytest.mark.parametrize("storage", ["two_lattice", "aa", "aax"])
+def test_single_slab_overlapped_through_the_comm_stream(storage):
     """world == 1 through SlabLbm.step(overlap=True): the exchange (self-periodic copies) runs on
     the second stream between begin and end."""
     import torch
@@ -233,10 +241,10 @@ def test_single_slab_overlapped_through_the_comm_stream():
     from paper_2206_15454_b200 import slab
 
     cfg = wl.small(nx=64, ny=8, nz=6)
-    ref = lb.Lbm.from_config(cfg, aa=False)
+    ref = lb.Lbm.from_config(cfg, aa={"two_lattice": False, "aa": True, "aax": "aax"}[storage])
     ref.init(3)
-    a = slab.SlabLbm(cfg, 0, 1)
-    b = slab.SlabLbm(cfg, 0, 1)
+    a = slab.SlabLbm(cfg, 0, 1, storage=storage)
+    b = slab.SlabLbm(cfg, 0, 1, storage=storage)
     a.init(3)
     b.init(3)
     ref.step(9)
