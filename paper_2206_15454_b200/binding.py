@@ -486,6 +486,25 @@ class Lbm:
         """Install a (19, nz, ny, nx) CUDA tensor of f_i - w_i as the plain state of step t."""
         _check(lib().lbm_set_state(self._h, self._dev(f_minus_w, (19,) + self.shape), int(t)))
 
+    def save_checkpoint(self, path: str):
+        """Write the plain state (lbm_get_state) and the time step to a file (plumbing: one device->host
+        copy and torch.save).  A run restarted with load_checkpoint continues bit for bit."""
+        import torch
+
+        # the momentum reference of the collision arithmetic is part of the bit-exact state
+        torch.save({"shape": self.shape, "t": self.time, "state": self.get_state().cpu(),
+                    "jx_ref": torch.from_numpy(self.get_reference_profile())}, path)
+
+    def load_checkpoint(self, path: str):
+        """Install a state written by save_checkpoint (lbm_set_state); the lattice shape must match."""
+        import torch
+
+        ck = torch.load(path, map_location="cpu")
+        if tuple(ck["shape"]) != tuple(self.shape):
+            raise ValueError(f"checkpoint is for a {ck['shape']} lattice, this handle is {self.shape}")
+        self.set_reference_profile(ck["jx_ref"].numpy())
+        self.set_state(ck["state"].to(self.device), int(ck["t"]))
+
     def diverged(self) -> bool:
         """True once lbm_get_macros* or the statistics reduction has seen a non-finite density."""
         flag = C.c_int(0)

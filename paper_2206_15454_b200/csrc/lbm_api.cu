@@ -64,7 +64,7 @@ static Layout make_layout(int nx, int ny, int nz, bool aa, bool mask)
     // partials per row: x chunks of the step launch (<= MAX_NCHUNK), TMA tiles, or - geometry handles - one
     // per warp of a row (KParams::wpart)
     int pmax = (nx / TMA_BOX > MAX_NCHUNK) ? nx / TMA_BOX : MAX_NCHUNK;
-    if (mask && (nx + 31) / 32 > pmax) pmax = (nx + 31) / 32;
+    if ((nx + 31) / 32 > pmax) pmax = (nx + 31) / 32;
     L.partial = off; off = align_up(off + (size_t)ny * NSTAT * nz * pmax * 4, 256);
     L.acc = off; off = align_up(off + (size_t)ny * NSTAT * 8, 256);
     L.shift = off; off = align_up(off + (size_t)ny * 4 * 4, 256);
@@ -171,7 +171,11 @@ static void set_variant(lbm_s *h)
 // The statistics partials are laid out with `pchunks` x chunks per row: the larger of the
 // chunkings of the kernels in use.  When it changes the buffer is cleared (entries no kernel
 // writes must read as zero in the stage-2 sum).
-static bool warp_partials(const lbm_s *h) { return h->mask && (h->TX % 32) == 0; }   // KParams::wpart
+static bool warp_partials(const lbm_s *h)   // KParams::wpart
+{
+    static const int all = [] { const char *e = getenv("LBM_WPART"); return (e && *e) ? atoi(e) : 0; }();   // A-B switch
+    return (h->mask || all) && (h->TX % 32) == 0;
+}
 static int want_pchunks(const lbm_s *h)
 {
     int pc = h->nchunk;

@@ -127,10 +127,19 @@ __device__ __forceinline__ void static_for(F &&f)
     }
 }
 
+// LBM_CS (build-time experiment switch, default 0): bit 0 = population loads with the streaming
+// cache hint (ld.global.cs), bit 1 = population stores with it (st.global.cs).
+#ifndef LBM_CS
+#define LBM_CS 0
+#endif
 template <int V> __device__ __forceinline__ void ldv(const float *p, float (&o)[V])
 {
     if constexpr (V == 4) {
+#if LBM_CS & 1
+        float4 t = __ldcs(reinterpret_cast<const float4 *>(p));
+#else
         float4 t = *reinterpret_cast<const float4 *>(p);
+#endif
         o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
     } else if constexpr (V == 2) {
         float2 t = *reinterpret_cast<const float2 *>(p);
@@ -141,7 +150,11 @@ template <int V> __device__ __forceinline__ void ldv(const float *p, float (&o)[
 }
 template <int V> __device__ __forceinline__ void stv(float *p, const float (&o)[V])
 {
+#if LBM_CS & 2
+    if constexpr (V == 4) __stcs(reinterpret_cast<float4 *>(p), make_float4(o[0], o[1], o[2], o[3]));
+#else
     if constexpr (V == 4) *reinterpret_cast<float4 *>(p) = make_float4(o[0], o[1], o[2], o[3]);
+#endif
     else if constexpr (V == 2) *reinterpret_cast<float2 *>(p) = make_float2(o[0], o[1]);
     else *p = o[0];
 }
@@ -167,6 +180,10 @@ __device__ __forceinline__ int block_index(const KParams &p)
 
 // `again`: recompute from laundered thread/block indices, so that the compiler does not keep the
 // first Ctx alive across the collision (register pressure of the AA odd step).
+// (A variant for launches with blockDim.y == 1 that drops threadIdx.y, so that the row and everything
+// derived from it becomes block-uniform and moves to the uniform datapath, was measured on cfg5: 7 %
+// fewer per-thread instructions, SM clock under the power cap 1635 instead of 1575 MHz, and 3.6 %
+// SLOWER - 40.1 against 41.6 GLUPS; the uniform pipe is the slower one.  Dropped.)
 template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0, bool again = false)
 {
     Ctx c;
@@ -909,6 +926,35 @@ template <int V, bool MASK> struct Bounds {
     static constexpr int minb = Occ<V>::minb;
 };
 
+// S2-S6 (+ the S8 sample) of the thread's V cells in registers: g holds the streamed populations on
+// entry and the post-collision ones on exit, s the thread's ten statistics sums.  Shared by the
+// per-thread and the TMA step kernels (bit-identical by construction).
+template <int V, bool STATS, bool MASK, bool SGS>
+__device__ __forceinline__ void cells_update(const KParams &p, float (&g)[Q][V], float (&s)[NSTAT], float cda,
+                                             unsigned fidx, float jr, unsigned long long S, int y)
+{
+    // (The same arithmetic on PAIRS of cells with Blackwell's packed fp32 instructions - FADD2 / FMUL2 /
+    // FFMA2, `__ffma2_rn` and friends: 105 instead of 243 fp32 instructions per cell - was built and
+    // measured in round 2: parity unchanged, but the pairs need 19 more live registers than the
+    // kernel has (40-140 B of spills with the statistics fused) and the kernel waits for DRAM, not
+    // for the fp32 pipe: cfg5 38.2 against 41.6 GLUPS with statistics, 41.4 against 42.5 without.  Dropped.)
+    if constexpr (STATS) {
+#pragma unroll
+        for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
+    }
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        mom_ref_shift<V>(g, k, jr);
+        const Cell m = moments<V>(p, g, k, cell_cda<MASK>(p, cda, fidx, k), jr);
+        if constexpr (STATS) {
+            // solid cells are left out of the plane sums (the divisor stays nx*nz, as in the
+            // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
+            if (!MASK || !((solid_self<V>(S) >> k) & 1u)) stats_add(s, m);
+        }
+        collide<V, SGS>(p, g, k, m, jr, y);
+    }
+}
+
 template <int V, int RM, int WM, bool STATS, bool MASK, bool SGS>
 __device__ __forceinline__ void step_body(const KParams &p)
 {
@@ -931,22 +977,15 @@ __device__ __forceinline__ void step_body(const KParams &p)
     const unsigned fidx = forest_idx<V, MASK>(p, c);
     const float jr = __ldg(p.jref + c.y);
     float s[NSTAT];
-    if constexpr (STATS) {
-#pragma unroll
-        for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
-    }
-#pragma unroll
-    for (int k = 0; k < V; ++k) {
-        mom_ref_shift<V>(g, k, jr);
-        const Cell m = moments<V>(p, g, k, cell_cda<MASK>(p, cda, fidx, k), jr);
-        if constexpr (STATS) {
-            // solid cells are left out of the plane sums (the divisor stays nx*nz, as in the
-            // oracle's O10); with a mask the host never sets an accumulation centre (p.shift)
-            if (!MASK || !((solid_self<V>(S) >> k) & 1u)) stats_add(s, m);
-        }
-        collide<V, SGS>(p, g, k, m, jr, c.y);
-    }
+    cells_update<V, STATS, MASK, SGS>(p, g, s, cda, fidx, jr, S, c.y);
     const Ctx c2 = (WM == WR_PUSH || WM == WR_XO) ? make_ctx<V>(p, p.z0 * p.ny, true) : c;
+    // the accumulation centre of the row is prefetched into L1 before the stores are issued and
+    // loaded after them: loaded where it is used its latency was 5-7 % of the warp time (ncu source
+    // page, round 2; the streaming loads keep evicting the small table from L1), and holding it in
+    // registers across the store phase spills in the x-balanced even step
+    if constexpr (STATS) {
+        if (p.shift) asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const float4 *>(p.shift) + c2.y));
+    }
     if (MASK && geom) store_all<V, WM, MASK>(p, c2, g, S);
     else store_all<V, WM, false>(p, c2, g);
     if constexpr (STATS) {

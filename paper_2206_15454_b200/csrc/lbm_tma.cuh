@@ -209,17 +209,7 @@ step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc)
 
     // ---- S2-S8 as in step_kernel ----
     float s[NSTAT];
-    if constexpr (STATS) {
-#pragma unroll
-        for (int k = 0; k < NSTAT; ++k) s[k] = 0.f;
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        mom_ref_shift<4>(g, k, jr);
-        const Cell m = moments<4>(p, g, k, cda, jr);
-        if constexpr (STATS) stats_add(s, m);
-        collide<4, false>(p, g, k, m, jr, c.y);
-    }
+    cells_update<4, STATS, false, false>(p, g, s, cda, 0u, jr, 0ull, c.y);
     const Ctx c2 = (WM == WR_PUSH) ? make_ctx<4>(p, p.z0 * p.ny, true) : c;
     store_all<4, WM, false>(p, c2, g);
     if constexpr (STATS) {

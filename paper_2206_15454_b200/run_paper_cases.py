@@ -4,7 +4,7 @@ profiles the paper plots: <u>/u_* (Fig. 10) and the stresses / u_*^2 (Fig. 11), 
 u_* = [<u'v'>^2 + <v'w'>^2]^(1/4) at y/h = 2 (L210).
 
     python -m paper_2206_15454_b200.run_paper_cases [--mesh fine|medium|coarse|small]
-           [--spinup N] [--window M] [--out report.md] [--boxes]
+           [--spinup N] [--window M] [--out report.md] [--boxes] [--sgs standard|damped|shear]
 
 Everything is computed by the CUDA library through its C ABI (lbm_step, lbm_stats_read,
 lbm_forest_friction_velocity, lbm_stats_normalise); this script only sequences the calls and
@@ -12,7 +12,11 @@ formats the table.  --boxes spins the flow up around 20-cell trip boxes near the
 them at run time before the averaging window (L226).  The comparison data of the paper's figures
 (field measurements, FVM LES) are not available here; what the text itself states is checked and
 reported: the near-ground velocity gradient of case 3 (no forest) exceeds that of cases 1 and 2
-(L289), and cases 1 and 2 differ only slightly (L305).
+(L289), and cases 1 and 2 differ only slightly (L305).  --sgs runs the same cases with one of the
+row-table SGS models (L307 "other SGS models"; lbm_set_sgs_rows): `damped` = van Driest wall damping
+of the Smagorinsky constant with u_tau = U_top / 12 (the balance the body force is derived from),
+`shear` = shear-improved Smagorinsky, the mean-shear table rebuilt from the running statistics every
+--refresh steps.
 """
 from __future__ import annotations
 
@@ -53,7 +57,22 @@ def trip_boxes(cfg: dict) -> np.ndarray:
     return m
 
 
-def run_case(lb, cfg: dict, spinup: int, window: int, boxes: bool, device="cuda:0"):
+def advance(lb, sim, n: int, sgs: str, refresh: int, top_wall: bool):
+    """n steps; with the shear-improved model the mean-shear table follows the running statistics."""
+    if sgs != "shear":
+        sim.step(n)
+        return
+    done = 0
+    while done < n:
+        k = min(refresh, n - done)
+        sim.step(k)
+        done += k
+        st, ns = sim.stats_read()
+        if ns > 0:
+            sim.set_sgs_rows(None, lb.sgs_mean_shear(st, top_wall=top_wall))
+
+
+def run_case(lb, cfg: dict, spinup: int, window: int, boxes: bool, device="cuda:0", sgs="standard", refresh=500):
     """(stats [ny][10], u_star, MLUPS) of one case."""
     import torch
 
@@ -64,15 +83,28 @@ def run_case(lb, cfg: dict, spinup: int, window: int, boxes: bool, device="cuda:
     if boxes:
         sim.set_solid(trip_boxes(cfg))
     sim.init(cfg["seed"])
-    sim.step(spinup)
+    top_wall = cfg["top"] == wl.BOUNCE_BACK
+    if sgs == "damped":
+        u_tau = cfg["init"]["U_ref"] / 12.0
+        sim.set_sgs_rows(lb.sgs_van_driest(cfg["ny"], cfg["Cs"], u_tau, cfg["nu"], 26.0, both_walls=top_wall), None)
+    if sgs == "shear":
+        sim.stats_accumulate(1)                   # the spin-up statistics feed the first tables
+    advance(lb, sim, spinup, sgs, refresh, top_wall)
     if boxes:
         sim.set_solid(None)                       # the boxes are removed, the flow is kept (L226)
-        sim.step(max(1, spinup // 4))
+        advance(lb, sim, max(1, spinup // 4), sgs, refresh, top_wall)
+    if sgs == "shear":
+        st, ns = sim.stats_read()
+        sim.set_sgs_rows(None, lb.sgs_mean_shear(st, top_wall=top_wall))
     sim.stats_accumulate(1)
     sim.stats_reset()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    sim.step(window)
+    if sgs == "shear":
+        # the table is frozen inside a refresh interval and follows the window's own running mean
+        advance(lb, sim, window, sgs, refresh, top_wall)
+    else:
+        sim.step(window)
     st, n = sim.stats_read()
     dt = time.perf_counter() - t0
     assert n == window
@@ -139,6 +171,9 @@ def main():
     ap.add_argument("--spinup", type=int, default=6000)
     ap.add_argument("--window", type=int, default=4000)
     ap.add_argument("--boxes", action="store_true", help="spin up around trip boxes, remove them at run time (L226)")
+    ap.add_argument("--sgs", choices=["standard", "damped", "shear"], default="standard",
+                    help="SGS closure: the paper's Smagorinsky model, or a row-table model (L307)")
+    ap.add_argument("--refresh", type=int, default=500, help="--sgs shear: steps between mean-shear table updates")
     ap.add_argument("--out", default=None, help="write the markdown report here (default: stdout)")
     args = ap.parse_args()
 
@@ -147,11 +182,12 @@ def main():
     cfgs = {k: case_config(args.mesh, k) for k in (1, 2, 3)}
     stats, ustar, mlups = {}, {}, {}
     for k in (1, 2, 3):
-        stats[k], ustar[k], mlups[k] = run_case(lb, cfgs[k], args.spinup, args.window, args.boxes)
+        stats[k], ustar[k], mlups[k] = run_case(lb, cfgs[k], args.spinup, args.window, args.boxes,
+                                                sgs=args.sgs, refresh=args.refresh)
     checks = text_checks(stats, cfgs[1]["h"])
     text = report(args.mesh, cfgs, stats, ustar, mlups, checks, lb)
     text += (f"\nRun: spin-up {args.spinup} steps, window {args.window} steps, trip boxes: {args.boxes}; "
-             "single-array AA storage, statistics every step.\n")
+             f"SGS model: {args.sgs}; single-array AA storage, statistics every step.\n")
     if args.out:
         os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
         with open(args.out, "w") as f:

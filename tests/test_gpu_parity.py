@@ -756,6 +756,32 @@ def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
     assert torch.equal(ra, rb) and torch.equal(ua, ub)
 
 
+@pytest.mark.parametrize("aa", [False, "aax"], ids=["pull2", "aax"])
+def test_checkpoint_file_restart_is_bit_identical(gpu, aa, tmp_path):
+    """save_checkpoint / load_checkpoint (lbm_get_state, lbm_set_state through a file): the restarted
+    run continues exactly like the uninterrupted one, from an odd and from an even time step."""
+    import torch
+    cfg = wl.small(nx=36, ny=10, nz=6)
+    a = gpu.Lbm.from_config(cfg, aa=aa)
+    a.init(11)
+    for t_save in (7, 20):
+        a.step(t_save - a.time)
+        path = str(tmp_path / f"ck{t_save}.pt")
+        a.save_checkpoint(path)
+        b = gpu.Lbm.from_config(cfg, aa=aa)
+        b.load_checkpoint(path)
+        assert b.time == t_save
+        a.step(9)
+        b.step(9)
+        torch.cuda.synchronize()
+        assert torch.equal(a.get_state(), b.get_state())
+        b.close()
+    c = gpu.Lbm.from_config(wl.small(nx=32, ny=10, nz=6), aa=aa)
+    with pytest.raises(ValueError):
+        c.load_checkpoint(path)
+    c.close(); a.close()
+
+
 @pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("t0", [0, 1])
 def test_p16_known_pi_neq_through_the_c_abi(orc, gpu, aa, t0):
