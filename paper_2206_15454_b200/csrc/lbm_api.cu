@@ -739,6 +739,10 @@ static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
     L.mask = h->mask && h->nflagged > 0;      // nothing flagged: the plain kernels
     L.aa = h->aa; L.aax = h->aax; L.odd = (h->t & 1) != 0;
     L.tma_mode = h->tma_mode; L.tma_rows = h->tma_rows;
+    {
+        static const int g3 = [] { const char *e = getenv("LBM_GRID3"); return (e && *e) ? atoi(e) : 1; }();   // A-B switch
+        L.grid3 = g3 != 0;
+    }
     // the map of the array this step reads (two-lattice: the roles swap every step)
     const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
     L.map = swapped ? &h->map_b : &h->map_a;

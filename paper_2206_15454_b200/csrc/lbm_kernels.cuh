@@ -109,6 +109,8 @@ struct KParams {
     unsigned long long seed;
     int z0, z1;                 // z range of a launch (chunked host transfers; interior planes of a slab)
     int rev;                    // 1 = the blocks walk the rows of the launch from the last to the first
+    int grid3;                  // 1 = 3-D grid (x chunk, row block of a plane, plane): the step launch when the
+                                //     block rows divide ny - no integer division in the index arithmetic
     int zg0, nzg;               // z slab: global z of local plane 0 and global nz (init recipe only)
     int zv0, zv1;               // planes that hold the lattice proper ([1, nz-1) on a z slab: not the ghosts)
     long long zoff;             // element offset of plane z0 inside rho_in/u_in/rho_out/u_out
@@ -177,6 +179,25 @@ __device__ __forceinline__ int block_index(const KParams &p)
 {
     return p.rev ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
 }
+// The same block order on a 3-D grid (blocks are dispatched x fastest, then y, then z): x = chunk of
+// the row, y = row block inside the plane, z = plane of the launch.  Saves the two integer divisions
+// (block -> row, row -> plane) of the 1-D form: ~55 of ~1450 instructions per thread.
+__device__ __forceinline__ void block_index3(const KParams &p, int &cb, int &yb, int &zb)
+{
+    cb = (int)blockIdx.x; yb = (int)blockIdx.y; zb = (int)blockIdx.z;
+    if (p.rev) { cb = (int)gridDim.x - 1 - cb; yb = (int)gridDim.y - 1 - yb; zb = (int)gridDim.z - 1 - zb; }
+}
+// index of the block in the whole-lattice order of the 1-D launch (per-block geometry flags)
+__device__ __forceinline__ long long block_linear(const KParams &p)
+{
+    const int rows_per_plane = p.ny / (int)blockDim.y;
+    if (p.grid3) {
+        int cb, yb, zb;
+        block_index3(p, cb, yb, zb);
+        return ((long long)(p.z0 + zb) * rows_per_plane + yb) * p.nchunk + cb;
+    }
+    return (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
+}
 
 // `again`: recompute from laundered thread/block indices, so that the compiler does not keep the
 // first Ctx alive across the collision (register pressure of the AA odd step).
@@ -187,17 +208,27 @@ __device__ __forceinline__ int block_index(const KParams &p)
 template <int V> __device__ __forceinline__ Ctx make_ctx(const KParams &p, int row0, bool again = false)
 {
     Ctx c;
-    int tx = threadIdx.x, ty = threadIdx.y, bx = block_index(p);
-    if (again) asm volatile("" : "+r"(tx), "+r"(ty), "+r"(bx));
+    int tx = threadIdx.x, ty = threadIdx.y;
+    if (p.grid3) {
+        int cb, yb, zb;
+        block_index3(p, cb, yb, zb);
+        if (again) asm volatile("" : "+r"(tx), "+r"(ty), "+r"(cb), "+r"(yb), "+r"(zb));
+        c.chunk = cb;
+        c.y = yb * (int)blockDim.y + ty;
+        c.z = p.z0 + zb;
+    } else {
+        int bx = block_index(p);
+        if (again) asm volatile("" : "+r"(tx), "+r"(ty), "+r"(bx));
+        // 1-D grid, the x chunks of a row are consecutive blocks (they run together, so the partial
+        // sectors at the chunk seams of the shifted stores merge in L2)
+        const int rb = bx / p.nchunk;
+        c.chunk = bx - rb * p.nchunk;
+        const int row = row0 + rb * blockDim.y + ty;
+        c.z = row / p.ny;
+        c.y = row - c.z * p.ny;
+    }
     const int lane = (ty * blockDim.x + tx) & 31;
-    // 1-D grid, the x chunks of a row are consecutive blocks (they run together, so the partial
-    // sectors at the chunk seams of the shifted stores merge in L2)
-    const int rb = bx / p.nchunk;
-    c.chunk = bx - rb * p.nchunk;
     c.x0 = (c.chunk * blockDim.x + tx) * V;
-    const int row = row0 + rb * blockDim.y + ty;
-    c.z = row / p.ny;
-    c.y = row - c.z * p.ny;
     c.xl = (c.x0 == 0) ? p.nx - 1 : c.x0 - 1;
     c.xr = (c.x0 + V >= p.nx) ? 0 : c.x0 + V;
     c.zm = (c.z == 0) ? p.nz - 1 : c.z - 1;
@@ -1009,8 +1040,7 @@ __global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::min
     // register allocation of the kernel without MASK, was measured: slower - cfg3 boxes + statistics
     // 39.2 against 39.7 GLUPS, cfg4 all-fluid mask -4.7 % against -0.7 % - and dropped.)
     if constexpr (MASK) {
-        const long long gb = (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
-        if (__ldg(p.bflag + gb) == 0) {
+        if (__ldg(p.bflag + block_linear(p)) == 0) {
             step_body<V, RM, WM, STATS, false, SGS>(p);
             return;
         }

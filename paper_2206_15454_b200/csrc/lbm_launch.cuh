@@ -19,6 +19,7 @@ struct StepLaunch {
     bool mask;               // geometry handle (solid mask / forest codes)
     bool aa, aax;            // single-array storage (AA, x-balanced AA); neither: two-lattice
     bool odd;                // time parity of the state the step reads
+    bool grid3;              // allow the 3-D grid form of the launch (A-B switch LBM_GRID3, default on)
     int tma_mode, tma_rows;  // TMA stream-in: step kinds (bit 0 AA even, 1 AA odd, 2 pull), rows per tile
     const CUtensorMap *map;  // tensor map of the array this step reads (TMA only)
     cudaStream_t stream;

@@ -11,9 +11,14 @@
 namespace lbm {
 
 template <int V, bool STATS, bool SGS>
-cudaError_t launch_step_t(const StepLaunch &L, const KParams &p)
+cudaError_t launch_step_t(const StepLaunch &L, const KParams &p0)
 {
-    dim3 block(L.TX, L.TY), grid((unsigned)((long long)(p.z1 - p.z0) * L.ny / L.TY * L.nchunk));
+    KParams p = p0;
+    const int planes = p.z1 - p.z0;
+    dim3 block(L.TX, L.TY), grid((unsigned)((long long)planes * L.ny / L.TY * L.nchunk));
+    // block rows that divide ny: the 3-D grid with the same block order (make_ctx: no divisions)
+    p.grid3 = (L.grid3 && L.ny % L.TY == 0 && L.ny / L.TY <= 65535 && planes <= 65535) ? 1 : 0;
+    if (p.grid3) grid = dim3((unsigned)L.nchunk, (unsigned)(L.ny / L.TY), (unsigned)planes);
     cudaStream_t st = L.stream;
     if (L.mask) {
         if (!L.aa) step_kernel<V, RD_PULL, WR_LOCAL, STATS, true, SGS><<<grid, block, 0, st>>>(p);
