@@ -42,9 +42,11 @@ BYTES_PER_CELL = 152.0  # 2 x 19 x 4 B (BASELINE.json:north_star; DESIGN.md "Roo
 # of the current kernels on the named config (profiles/): the line quotes the figure of its own
 # config when one exists, else null.
 NCU_TRAFFIC_BYTES_PER_CELL = {
-    ("cfg5", "aa"): (152.1, "profiles/r02_README.md, ncu dram__bytes_read+write on cfg5 itself, both AA parities"),
-    ("cfg4", "aa"): (151.7, "profiles/r02_README.md, ncu --set full on cfg4, both AA parities"),
-    ("cfg3", "two_lattice"): (149.0, "profiles/r01_README.md, ncu --set full on cfg3"),
+    ("cfg5", "aax"): (152.11, "profiles/r02_dram_cfg5.csv, ncu dram__bytes_read+write on cfg5 itself, both parities"),
+    ("cfg4", "aax"): (151.7, "profiles/r02_step_kernel_cfg4_details.txt, ncu --set full on cfg4, both parities"),
+    ("cfg3", "two_lattice"): (149.1, "profiles/r02_step_kernel_cfg3_stats_details.txt, ncu --set full on cfg3"),
+    ("cfg2", "aax"): (138.8, "profiles/r02_step_kernel_cfg2_details.txt, ncu --set full on cfg2 (part of the writes "
+                             "is still dirty in the L2 when the launch ends)"),
 }
 METRIC = "MLUPS"
 UNIT = "MLUPS (1e6 lattice-cell updates/s)"
