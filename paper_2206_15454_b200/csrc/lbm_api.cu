@@ -730,6 +730,12 @@ static cudaError_t launch_macros(lbm_s *h, const KParams &p, int planes)
     }
 }
 
+static bool pdl_enabled()
+{
+    static const int on = [] { const char *e = getenv("LBM_PDL"); return (e && *e) ? atoi(e) : 1; }();   // A-B switch
+    return on != 0;
+}
+
 // One launch of the fused step for the planes [p.z0, p.z1): the launchers live in their own
 // translation units (lbm_launch.cuh), one per (cells per thread, statistics, SGS row table).
 static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
@@ -742,6 +748,7 @@ static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
     {
         static const int g3 = [] { const char *e = getenv("LBM_GRID3"); return (e && *e) ? atoi(e) : 1; }();   // A-B switch
         L.grid3 = g3 != 0;
+        L.pdl = pdl_enabled();
     }
     // the map of the array this step reads (two-lattice: the roles swap every step)
     const bool swapped = !h->aa && p.src != reinterpret_cast<float *>(h->ws + h->L.pops);
@@ -767,12 +774,11 @@ static cudaError_t launch_step(lbm_s *h, const KParams &p, bool stats)
 static cudaError_t launch_stage2(lbm_s *h, int mode)
 {
     dim3 grid(h->ny, NSTAT);
-    stats_stage2_kernel<<<grid, 256, 0, h->stream>>>(
+    h->launches++;
+    return launch_chain(stats_stage2_kernel, grid, dim3(256), 0, h->stream, pdl_enabled(),
         reinterpret_cast<const float *>(h->ws + h->L.partial), (long long)h->nz * h->pchunks,
         reinterpret_cast<double *>(h->ws + h->L.acc), reinterpret_cast<float *>(h->ws + h->L.shift), mode,
         1.0 / ((double)h->nx * h->nz), reinterpret_cast<int *>(h->ws + h->L.flag));
-    h->launches++;
-    return cudaGetLastError();
 }
 
 static int stats_reset_impl(lbm_s *h)

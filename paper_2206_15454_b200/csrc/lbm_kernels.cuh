@@ -199,6 +199,16 @@ __device__ __forceinline__ long long block_linear(const KParams &p)
     return (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
 }
 
+// Programmatic dependent launch (lbm_launch.cuh: launch_chain): wait until the preceding launch of the
+// chain has completed and its writes are visible, then let the following launch be set up.  Both are
+// no-ops for a kernel that was launched without the attribute.  Must run before the first access to
+// anything a preceding kernel wrote.
+__device__ __forceinline__ void pdl_enter()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // `again`: recompute from laundered thread/block indices, so that the compiler does not keep the
 // first Ctx alive across the collision (register pressure of the AA odd step).
 // (A variant for launches with blockDim.y == 1 that drops threadIdx.y, so that the row and everything
@@ -1036,6 +1046,7 @@ __device__ __forceinline__ void step_body(const KParams &p)
 template <int V, int RM, int WM, bool STATS, bool MASK = false, bool SGS = false>
 __global__ void __launch_bounds__(Bounds<V, MASK>::threads, Bounds<V, MASK>::minb) step_kernel(const KParams p)
 {
+    pdl_enter();
     // (The geometry body as a __noinline__ function of its own, so that the plain body keeps the
     // register allocation of the kernel without MASK, was measured: slower - cfg3 boxes + statistics
     // 39.2 against 39.7 GLUPS, cfg4 all-fluid mask -4.7 % against -0.7 % - and dropped.)
@@ -1332,6 +1343,7 @@ static __global__ void __launch_bounds__(256) stats_stage2_kernel(const float *_
                                                            double inv_count, int *diverged)
 {
     __shared__ double sm[8];
+    pdl_enter();
     const int y = blockIdx.x, k = blockIdx.y;
     const float *src = partial + ((long long)y * NSTAT + k) * len;
     double t = 0.0;

@@ -20,10 +20,29 @@ struct StepLaunch {
     bool aa, aax;            // single-array storage (AA, x-balanced AA); neither: two-lattice
     bool odd;                // time parity of the state the step reads
     bool grid3;              // allow the 3-D grid form of the launch (A-B switch LBM_GRID3, default on)
+    bool pdl;                // programmatic dependent launch (A-B switch LBM_PDL, default on)
     int tma_mode, tma_rows;  // TMA stream-in: step kinds (bit 0 AA even, 1 AA odd, 2 pull), rows per tile
     const CUtensorMap *map;  // tensor map of the array this step reads (TMA only)
     cudaStream_t stream;
 };
+
+// Kernel launch with the programmatic-stream-serialization attribute (programmatic dependent launch):
+// the step kernels and the statistics stage 2 start with griddepcontrol.wait + launch_dependents
+// (lbm_kernels.cuh: pdl_enter), so the NEXT launch of the chain is set up on the SMs while the last
+// wave of this one is still running and starts the moment its predecessor has completed and flushed -
+// the launch latency, which is what bounds lattices of a few 10^5 cells (cfg1: a 3 us kernel), hides.
+template <class... KArgs, class... Args>
+inline cudaError_t launch_chain(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
 
 // One launch of step_kernel<V, RM, WM, STATS, MASK, SGS> for the planes [p.z0, p.z1).
 template <int V, bool STATS, bool SGS>

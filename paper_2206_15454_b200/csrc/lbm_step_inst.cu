@@ -21,15 +21,14 @@ cudaError_t launch_step_t(const StepLaunch &L, const KParams &p0)
     if (p.grid3) grid = dim3((unsigned)L.nchunk, (unsigned)(L.ny / L.TY), (unsigned)planes);
     cudaStream_t st = L.stream;
     if (L.mask) {
-        if (!L.aa) step_kernel<V, RD_PULL, WR_LOCAL, STATS, true, SGS><<<grid, block, 0, st>>>(p);
-        else if (!L.odd) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, true, SGS><<<grid, block, 0, st>>>(p);
-        else step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, true, SGS><<<grid, block, 0, st>>>(p);
-    } else if (!L.aa) step_kernel<V, RD_PULL, WR_LOCAL, STATS, false, SGS><<<grid, block, 0, st>>>(p);
-    else if (L.aax && !L.odd) step_kernel<V, RD_XE, WR_XE, STATS, false, SGS><<<grid, block, 0, st>>>(p);
-    else if (L.aax) step_kernel<V, RD_XO, WR_XO, STATS, false, SGS><<<grid, block, 0, st>>>(p);
-    else if (!L.odd) step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, false, SGS><<<grid, block, 0, st>>>(p);
-    else step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, false, SGS><<<grid, block, 0, st>>>(p);
-    return cudaGetLastError();
+        if (!L.aa) return launch_chain(step_kernel<V, RD_PULL, WR_LOCAL, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
+        else if (!L.odd) return launch_chain(step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
+        else return launch_chain(step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
+    } else if (!L.aa) return launch_chain(step_kernel<V, RD_PULL, WR_LOCAL, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);
+    else if (L.aax && !L.odd) return launch_chain(step_kernel<V, RD_XE, WR_XE, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);
+    else if (L.aax) return launch_chain(step_kernel<V, RD_XO, WR_XO, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);
+    else if (!L.odd) return launch_chain(step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);
+    else return launch_chain(step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);
 }
 
 template cudaError_t launch_step_t<LBM_V, (LBM_S != 0), (LBM_G != 0)>(const StepLaunch &, const KParams &);

@@ -136,6 +136,7 @@ step_tma_kernel(const KParams p, const __grid_constant__ CUtensorMap msrc)
     float *halo = buf + Q * R * TMA_BOX;                 // [Q][R]
     __shared__ __align__(8) uint64_t bar;
 
+    pdl_enter();
     const Ctx c = make_ctx<4>(p, p.z0 * p.ny);
     const int tx = threadIdx.x, ty = threadIdx.y, lin = ty * TMA_TX + tx;
     const int x0t = c.chunk * TMA_BOX;

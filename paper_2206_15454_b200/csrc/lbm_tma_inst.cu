@@ -22,8 +22,7 @@ static cudaError_t launch_tma_r(const StepLaunch &L, const KParams &p0)
     KParams p = p0;
     p.nchunk = L.nx / TMA_BOX;                   // tiles per row (make_ctx decomposes the block index with it)
     dim3 block(TMA_TX, R), grid((unsigned)((long long)(p.z1 - p.z0) * L.ny / R * p.nchunk));
-    step_tma_kernel<RM, WM, S, R><<<grid, block, smem, L.stream>>>(p, *L.map);
-    return cudaGetLastError();
+    return launch_chain(step_tma_kernel<RM, WM, S, R>, grid, block, (size_t)smem, L.stream, L.pdl, p, *L.map);
 }
 template <int RM, int WM, bool S>
 static cudaError_t launch_tma_rows(const StepLaunch &L, const KParams &p)
