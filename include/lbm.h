@@ -326,6 +326,18 @@ int lbm_set_sweep(lbm_t *h, int mode);
 int lbm_set_kernel_timing(lbm_t *h, int on);
 int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches);
 
+/* Environment variables the library reads (measurement switches; none changes a result):
+ *   LBM_STAGING_BYTES  size of the host-transfer staging area (default 256 MB), read at every call
+ *   LBM_TMA="m[,r]"    default of lbm_set_tma for new handles (default 0: per-thread loads)
+ *   LBM_SWEEP=0|1      default of lbm_set_sweep for new handles (default 1: alternating direction)
+ *   LBM_GRID3=0|1      step launch on a 3-D grid (x chunk, row block, plane; default 1) or on the 1-D
+ *                      grid whose index arithmetic needs two integer divisions; read once per process
+ *   LBM_PDL=0|1        programmatic dependent launch of the step / statistics kernels (default 1);
+ *                      read once per process
+ *   LBM_WPART=0|1      per-warp statistics partials for every handle, not only geometry handles
+ *                      (default 0); read once per process
+ * DESIGN.md "Kernels" and profiles/r02_README.md give the A/B numbers behind the defaults. */
+
 /* Name of the kernel variant lbm_step uses, e.g. "aa/v4/tx384x1" (static string per handle). */
 const char *lbm_variant(const lbm_t *h);
 

@@ -87,3 +87,25 @@ def test_gpu_cases_agree_with_the_oracle(orc, oracle_cases, aa):
         g.close()
     ck = text_checks(stats, 7)
     assert ck["case3_gradient_largest"] and ck["case3_near_ground_u_largest"] and ck["cases_1_2_differ_slightly"]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("sgs", ["damped", "shear"])
+def test_runner_with_row_table_sgs_models(sgs):
+    """run_paper_cases.run_case with the row-table SGS models on the oracle-sized ABL:
+    finite statistics, a positive friction velocity, and what the text says about the three cases
+    (L283-305) still holds; the shear-improved run refreshes its table from the running statistics."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200.run_paper_cases import run_case
+    stats = {}
+    for k in (1, 2, 3):
+        cfg = wl.abl_case_small(k)
+        st, us, mlups = run_case(lb, cfg, SPINUP, WINDOW, boxes=False, sgs=sgs, refresh=100)
+        assert np.isfinite(st).all() and mlups > 0
+        assert k == 3 or us > 0
+        stats[k] = st
+    ck = text_checks(stats, 7)
+    assert ck["case3_gradient_largest"] and ck["case3_near_ground_u_largest"] and ck["cases_1_2_differ_slightly"]
