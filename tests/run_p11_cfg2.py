@@ -4,7 +4,8 @@ the CUDA path and on the fp64 oracle from the same seeded field; plus a second C
 another seed as the sampling-noise floor (SURVEY.md §7 hard part 11).
 
 Not a pytest test (the oracle side takes about an hour on 16 cores):
-    python tests/run_p11_cfg2.py [--spin 20000] [--window 20000] [--out gpurun_out/p11_cfg2.md]
+    python tests/run_p11_cfg2.py [--spin 20000] [--window 20000] [--storage aax|aa|two_lattice]
+                                 [--out gpurun_out/p11_cfg2.md]
 The report is rewritten every `--every` window steps so that a cut-off run still leaves numbers.
 north_star bar: plane-averaged mean within 2 %, Reynolds stresses within 5 % (of the profile maxima).
 """
@@ -39,13 +40,17 @@ def main():
     ap.add_argument("--spin", type=int, default=20000)
     ap.add_argument("--window", type=int, default=20000)
     ap.add_argument("--every", type=int, default=2500)
+    ap.add_argument("--storage", choices=["aax", "aa", "two_lattice"], default=None,
+                    help="storage scheme of the CUDA runs (default: the config's)")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "p11_cfg2.md"))
     args = ap.parse_args()
     cfg = wl.get("cfg2")
+    if args.storage:
+        cfg["storage"] = args.storage
     t0 = time.time()
 
     def gpu_run(seed):
-        g = lb.Lbm.from_config(cfg, aa=False)
+        g = lb.Lbm.from_config(cfg)            # storage scheme from cfg["storage"]
         g.init(seed)
         g.step(args.spin)
         g.stats_accumulate(1)
@@ -72,7 +77,7 @@ def main():
         d_par, d_floor = diffs(sa, so), diffs(sb, sa)
         lines = [
             "# P11 — config 2 long-run statistical parity (CUDA path vs fp64 oracle)", "",
-            f"Command: `python tests/run_p11_cfg2.py --spin {args.spin} --window {args.window}` on one B200 "
+            f"Command: `python tests/run_p11_cfg2.py --spin {args.spin} --window {args.window} --storage {cfg['storage']}` on one B200 "
             f"+ {os.cpu_count()} host cores; lattice {cfg['nx']}x{cfg['ny']}x{cfg['nz']}, seed {cfg['seed']}; "
             f"variant {ga.variant}.", "",
             f"Window so far: {done} of {args.window} steps after {args.spin} spin-up steps "

@@ -9,7 +9,8 @@ percentages are read in DESIGN.md §4 ("of the profile maximum"), and additional
 relative to the local value wherever the profile exceeds a fifth of its maximum (near zero
 crossings a relative bound means nothing).  Lattices are the ones the oracle finishes in seconds:
 these are small-lattice, short-window checks; the full-length config-2 run (20 k + 20 k steps, one
-hour of oracle time) is tests/run_p11_cfg2.py, its report profiles/r01_p11_cfg2.md.
+hour of oracle time) is tests/run_p11_cfg2.py, its reports profiles/r01_p11_cfg2.md (round 1,
+two-lattice) and profiles/r02_p11_cfg2.md (round 2, the final x-balanced AA kernels).
 """
 import numpy as np
 import pytest
