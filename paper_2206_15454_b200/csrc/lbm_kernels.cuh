@@ -1378,9 +1378,16 @@ static __global__ void __launch_bounds__(256) stats_stage2_kernel(const float *_
 // ghost plane has written may land: an entry whose source cell lies beyond a wall / lid face or is
 // solid holds the destination cell's own bounced population and stays; nothing lands in a solid cell.
 // ---------------------------------------------------------------------------------------------
+// One launch serves one face (gridDim.y = 1) or both (gridDim.y = 2: blockIdx.y = 1 takes the
+// second (z, side, buf) triple).
+struct HaloFace { int z, side; float *buf; };
 template <bool PACK, bool FILTER>
-__global__ void halo_kernel(const KParams p, float *pops, int z, int side, float *buf)
+__global__ void halo_kernel(const KParams p, float *pops, HaloFace f0, HaloFace f1)
 {
+    pdl_enter();
+    const HaloFace f = blockIdx.y ? f1 : f0;
+    const int z = f.z, side = f.side;
+    float *buf = f.buf;
     const long long plane = (long long)p.nx * p.ny;
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= 5 * plane) return;
