@@ -264,7 +264,7 @@ def run_b200(args, cfg):
     K, W = args.steps, args.warmup
     N = wl.n_cells(cfg)
     every = cfg.get("stats_every", 0)
-    sim = lb.Lbm.from_config(cfg, device=dev)          # storage scheme from cfg["storage"]
+    sim = lb.Lbm.from_config(cfg, vec=args.vec, device=dev)   # storage scheme from cfg["storage"]
     if args.shape:
         tx, ty = (int(v) for v in args.shape.split("x"))
         sim.set_launch_shape(tx, ty)
@@ -518,6 +518,8 @@ def main():
     ap.add_argument("--shape", default=None, help="thread-block shape override TXxTY (tuning)")
     ap.add_argument("--tma", default=None,
                     help="A/B: step kinds on the TMA path, 'mode[,rows]' (bit 0 AA even, 1 AA odd, 2 pull)")
+    ap.add_argument("--vec", type=int, choices=[0, 1, 2, 4], default=0,
+                    help="A/B: cells per thread (0 = the library's choice)")
     ap.add_argument("--sweep", type=int, choices=[0, 1], default=None,
                     help="A/B: 0 = every step walks the lattice forward, 1 = alternating direction (default)")
     ap.add_argument("--traffic", type=float, default=None,

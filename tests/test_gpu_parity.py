@@ -694,7 +694,7 @@ def test_masked_update_is_run_to_run_bit_identical(gpu, aa):
             cfg["solid"] = (rng.random((12, 16, 96)) < 0.15).astype(np.uint8)
         ref = None
         for rep in range(5):
-            g = gpu.Lbm.from_config(cfg, aa=aa)
+            g = gpu.Lbm.from_config(cfg, aa=aa, vec=4)
             g.set_launch_shape(*[(24, 4), (8, 16), (12, 8), (24, 8), (6, 2)][rep]) if not solid else None
             g.init(cfg["seed"])
             g.stats_accumulate(1)
@@ -982,8 +982,8 @@ def test_tma_path_is_bit_identical_to_the_per_thread_path(orc, gpu, aa, rows, nx
     cfg = wl.small(nx=nx, ny=8, nz=5, bottom=bottom, top=top)
     if top == wl.FORCED_EQ:
         cfg["U_top"] = (0.06, 0.0, 0.01)
-    a = gpu.Lbm.from_config(cfg, aa=aa)
-    b = gpu.Lbm.from_config(cfg, aa=aa)
+    a = gpu.Lbm.from_config(cfg, aa=aa, vec=4)       # (lattices this small default to 1 cell per thread)
+    b = gpu.Lbm.from_config(cfg, aa=aa, vec=4)
     a.set_tma(0)
     b.set_tma(7, rows)
     assert "tma" not in a.variant and f"tma7x{rows}" in b.variant
@@ -1007,12 +1007,13 @@ def test_tma_path_is_bit_identical_to_the_per_thread_path(orc, gpu, aa, rows, nx
 
 
 def test_tma_is_refused_where_it_cannot_run(gpu):
-    g = gpu.Lbm(64, 4, 4, 0.01, 0.1)
+    v4 = gpu.bc_flags("bounce_back", "bounce_back", vec=4)
+    g = gpu.Lbm(64, 4, 4, 0.01, 0.1, flags=v4)
     with pytest.raises(gpu.LbmError) as e:
         g.set_tma(2)
     assert e.value.code == gpu.LBM_EINVAL
     g.set_tma(0)
-    g = gpu.Lbm(256, 6, 4, 0.01, 0.1)
+    g = gpu.Lbm(256, 6, 4, 0.01, 0.1, flags=v4)
     with pytest.raises(gpu.LbmError):
         g.set_tma(7, 4)                      # 4 rows do not divide ny = 6
     g.set_tma(7, 2)
