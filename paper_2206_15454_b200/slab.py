@@ -56,7 +56,7 @@ class SlabLbm:
     torch.distributed's default group (world == 1: the slab is its own neighbour)."""
 
     def __init__(self, cfg: dict, rank: int = 0, world: int = 1, device="cuda:0", group=None,
-                 emulated: bool = False, storage: str = "two_lattice"):
+                 emulated: bool = False, storage: str = "two_lattice", vec: int = 0):
         if cfg["nz"] % world:
             raise ValueError(f"nz={cfg['nz']} is not a multiple of the number of slabs {world}")
         self.rank, self.world, self.group = int(rank), int(world), group
@@ -72,7 +72,7 @@ class SlabLbm:
         if storage not in ("two_lattice", "aa", "aax"):
             raise ValueError(f"unknown storage scheme {storage!r}")
         aa = {"two_lattice": False, "aa": True, "aax": "aax"}[storage]
-        self.sim = Lbm.from_config(local, aa=aa, halo=True, device=device)
+        self.sim = Lbm.from_config(local, aa=aa, vec=vec, halo=True, device=device)
         self.sim.set_z_slab(self.z_first, self.nz_global)
         self.cfg = cfg
         self._send = [self.sim.halo_buffer(), self.sim.halo_buffer()]    # [lo, hi]

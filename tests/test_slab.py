@@ -105,11 +105,12 @@ def test_emulated_slabs_equal_global_lattice(world, case, storage):
         m[2:4, 7:10, 12:15] = True                       # ... and one under the top face, across a slab face
         cfg["solid"] = m
     aa = {"two_lattice": False, "aa": True, "aax": "aax"}[storage]
-    ref = lb.Lbm.from_config(cfg, aa=aa)
+    vec = 4 if world % 2 == 0 else 0        # 4 cells per thread and the small-lattice default (1)
+    ref = lb.Lbm.from_config(cfg, aa=aa, vec=vec)
     ref.init(cfg["seed"])
     ref.stats_accumulate(1)
     ref.stats_reset()
-    slabs = [slab.SlabLbm(cfg, r, world, emulated=True, storage=storage) for r in range(world)]
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True, storage=storage, vec=vec) for r in range(world)]
     slab.init_emulated(slabs, cfg["seed"])
     for s in slabs:
         s.stats_accumulate(1)
