@@ -326,6 +326,25 @@ int lbm_set_sweep(lbm_t *h, int mode);
 int lbm_set_kernel_timing(lbm_t *h, int on);
 int lbm_kernel_timing_read(lbm_t *h, double *total_ms, long long *launches);
 
+/* Plane statistics of ONE sample given as fields, with NO allocation of any kind (no cudaMalloc,
+ * cudaFree, or allocating library call; no handle, no workspace) - for callers that cannot allocate:
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid it.  The two-stage
+ * reduction of the statistics path (S8, S9) over x and z:
+ *   rho_dev  device, [nz][ny][nx] fp32;  u_dev  device, [3][nz][ny][nx] fp32 (as lbm_get_macros writes)
+ *   out_dev  device, [ny][LBM_NSTAT] doubles, the columns of lbm_stats_read for this one sample:
+ *            <u>,<v>,<w>,<u'u'>,<v'v'>,<w'w'>,<u'v'>,<v'w'>,<u'w'>,<rho>, averages over the x-z plane
+ * Asynchronous on cuda_stream (a cudaStream_t passed as void*, NULL = the default stream), on the
+ * device that owns rho_dev.  The stage-1 row sums go through a scratch array of
+ * LBM_STATIC_SCRATCH_BYTES that is part of the library image: every GPU that loads the library holds
+ * it until the process exits.  Limit: 10 * 4 * ny * nz bytes must fit, i.e. ny*nz <= 419 430 rows
+ * (and nz <= 65 535) - config 5 (384 x 1024) fits; LBM_EINVAL with the numbers in lbm_last_error()
+ * otherwise.  Every call shares that array, which keeps the last call's contents (nothing needs to
+ * start at zero: each call writes all it reads): calls that OVERLAP on the GPU - different streams,
+ * different threads - race on it; calls on one stream are safe.  LBM_ECUDA on a CUDA error. */
+#define LBM_STATIC_SCRATCH_BYTES (16 * 1024 * 1024)
+int lbm_plane_stats_static(const float *rho_dev, const float *u_dev, int nx, int ny, int nz,
+                           double *out_dev, void *cuda_stream);
+
 /* Environment variables the library reads (measurement switches; none changes a result):
  *   LBM_STAGING_BYTES  size of the host-transfer staging area (default 256 MB), read at every call
  *   LBM_TMA="m[,r]"    default of lbm_set_tma for new handles (default 0: per-thread loads)

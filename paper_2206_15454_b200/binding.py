@@ -43,7 +43,7 @@ SYMBOLS = [
     "lbm_forest_friction_velocity", "lbm_stats_normalise", "lbm_wall_units", "lbm_set_graphs", "lbm_set_z_slab",
     "lbm_halo_bytes", "lbm_halo_pack", "lbm_halo_unpack", "lbm_stats_read_raw", "lbm_stats_from_raw",
     "lbm_set_state", "lbm_diverged", "lbm_set_reference_profile", "lbm_get_reference_profile", "lbm_set_tma", "lbm_set_sweep",
-    "lbm_set_sgs_rows", "lbm_sgs_van_driest", "lbm_sgs_mean_shear",
+    "lbm_set_sgs_rows", "lbm_sgs_van_driest", "lbm_sgs_mean_shear", "lbm_plane_stats_static",
     "lbm_set_forest_codes", "lbm_forest_code", "lbm_lad_eq14", "lbm_step_slab_begin", "lbm_step_slab_end",
 ]
 
@@ -106,6 +106,7 @@ def lib():
         L.lbm_set_sgs_rows.argtypes = [vp, vp, vp]
         L.lbm_sgs_van_driest.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp]
         L.lbm_sgs_mean_shear.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.lbm_plane_stats_static.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp]
         L.lbm_time.argtypes = [vp]
         L.lbm_time.restype = C.c_longlong
         L.lbm_launch_count.argtypes = [vp]
@@ -195,6 +196,30 @@ def stats_from_raw(raw: np.ndarray, count: float, centre=None) -> np.ndarray:
     out = np.empty_like(raw)
     cp = None if centre is None else _dp(np.ascontiguousarray(centre, dtype=np.float64))
     _check(lib().lbm_stats_from_raw(_dp(raw), cp, raw.shape[0], float(count), _dp(out)))
+    return out
+
+
+STATIC_SCRATCH_BYTES = 16 * 1024 * 1024   # LBM_STATIC_SCRATCH_BYTES of include/lbm.h
+
+
+def plane_stats_static(rho, u, out=None, stream=None, shape=None):
+    """lbm_plane_stats_static: plane statistics of one (rho, u) sample without any allocation inside
+    the library (its scratch is a static device array).  rho (nz, ny, nx), u (3, nz, ny, nx): CUDA
+    float32 tensors; out: a CUDA float64 tensor (ny, NSTAT), made here when None (the caller's
+    allocation, not the library's).  `shape` = (nz, ny, nx) overrides the tensors' shape (tests of
+    the size check).  Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+
+    nz, ny, nx = shape if shape is not None else rho.shape
+    if out is None:
+        out = torch.empty((ny, NSTAT), dtype=torch.float64, device=rho.device)
+    if stream is None:
+        stream = torch.cuda.current_stream(rho.device)
+    for t, dt in ((rho, torch.float32), (u, torch.float32), (out, torch.float64)):
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise ValueError("plane_stats_static needs contiguous CUDA tensors: rho, u float32, out float64")
+    _check(lib().lbm_plane_stats_static(C.c_void_p(rho.data_ptr()), C.c_void_p(u.data_ptr()), int(nx), int(ny), int(nz),
+                                        C.c_void_p(out.data_ptr()), C.c_void_p(stream.cuda_stream)))
     return out
 
 

@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 OBJ = os.path.join(_HERE, "build")
-DEPS = [os.path.join(CSRC, f) for f in ("lbm_api.cu", "lbm_step_inst.cu", "lbm_tma_inst.cu", "lbm_kernels.cuh",
+DEPS = [os.path.join(CSRC, f) for f in ("lbm_api.cu", "lbm_static.cu", "lbm_step_inst.cu", "lbm_tma_inst.cu", "lbm_kernels.cuh",
                                          "lbm_tma.cuh", "lbm_launch.cuh")] + [os.path.join(ROOT, "include", "lbm.h")]
 LIB = os.path.join(_HERE, "liblbm_b200.so")
 
@@ -38,7 +38,7 @@ NVCC_FLAGS = [
 
 def units():
     """(object name, source, extra defines) of every translation unit."""
-    out = [("lbm_api.o", "lbm_api.cu", [])]
+    out = [("lbm_api.o", "lbm_api.cu", []), ("lbm_static.o", "lbm_static.cu", [])]
     for v in (4, 2, 1):
         for s in (0, 1):
             for g in (0, 1):
@@ -71,7 +71,7 @@ def _stale(obj: str, src: str) -> bool:
             os.path.abspath(__file__)]
     if src == "lbm_tma_inst.cu":
         deps.append(os.path.join(CSRC, "lbm_tma.cuh"))
-    if src == "lbm_api.cu":
+    if src in ("lbm_api.cu", "lbm_static.cu"):
         deps.append(os.path.join(ROOT, "include", "lbm.h"))
     t = os.path.getmtime(o)
     return any(os.path.getmtime(d) > t for d in deps)

@@ -25,6 +25,9 @@ static int fail(int code, const char *fmt, ...)
     return code;
 }
 
+// for the other translation units of the library (lbm_static.cu): set the text of lbm_last_error()
+int lbm_fail_msg(int code, const char *msg) { return fail(code, "%s", msg); }
+
 #define CU_TRY(expr)                                                                          \
     do {                                                                                      \
         cudaError_t e__ = (expr);                                                             \
