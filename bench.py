@@ -552,8 +552,6 @@ def main():
     if args.geometry:
         cfg["geometry"] = True
         cfg["note"] += ", geometry handle with an all-fluid mask"
-    if (args.boxes or args.geometry) and cfg["storage"] == "aax":
-        cfg["storage"] = "aa"          # the geometry variants exist for the two-lattice and AA storage
     if args.impl == "reference":
         return run_reference(args, cfg)
     if args.sharded:

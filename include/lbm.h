@@ -68,7 +68,7 @@ typedef enum lbm_status {
 #define LBM_VEC_MASK          (7u << 8)
 #define LBM_STORAGE_AAX       (1u << 11)  /* bit 11: single array, x-balanced AA pattern: as LBM_STORAGE_AA in
                                              memory and results, but both steps of the pattern carry half of
-                                             the x streaming (lbm_kernels.cuh "AAX"); no LBM_SOLID_MASK       */
+                                             the x streaming (lbm_kernels.cuh "AAX"); geometry handles too     */
 
 #define LBM_NSTAT 10 /* columns of lbm_stats_read */
 

@@ -282,8 +282,6 @@ int lbm_create(lbm_t **out, int nx, int ny, int nz, double nu, double Cs, const 
         return fail(LBM_EINVAL, "unknown bits in bc_flags 0x%x", bc_flags);
     int bot, top;
     if (!valid_top_bottom(bc_flags, &bot, &top)) return fail(LBM_EINVAL, "unsupported boundary combination in bc_flags 0x%x", bc_flags);
-    if ((bc_flags & LBM_STORAGE_AAX) && (bc_flags & LBM_SOLID_MASK))
-        return fail(LBM_EINVAL, "LBM_STORAGE_AAX has no geometry variant: use LBM_STORAGE_AA or two-lattice storage with LBM_SOLID_MASK");
     if (bc_flags & LBM_Z_HALO) {
         if (nz < 3) return fail(LBM_EINVAL, "LBM_Z_HALO needs nz >= 3 (two ghost planes + >= 1 interior)");
     }
@@ -394,6 +392,7 @@ static void fill_params(lbm_s *h)
     p.jref = reinterpret_cast<const float *>(h->ws + h->L.jref);
     p.sgs = h->sgs_rows ? reinterpret_cast<const float2 *>(h->ws + h->L.sgs) : nullptr;
     p.bot = h->bot; p.top = h->top; p.drag_vector = h->drag_vector ? 1 : 0;
+    p.aax = h->aax ? 1 : 0;
     {
         // lid populations f_eq,i(1, U_top) - w_i (Eq. 3) of the five directions with c_y = -1
         static const int li[5] = {4, 8, 9, 16, 18};
@@ -579,7 +578,11 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
         KParams p = h->kp;
         float *arr = (!h->aa && (h->t & 1)) ? p.dst : p.src;            // the array holding state t
         const unsigned blocks = (unsigned)((h->N + 255) / 256);
-        if (h->aa && (h->t & 1) == 0)
+        if (h->aax && (h->t & 1) == 0)
+            mask_change_kernel<true, true><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
+        else if (h->aax)
+            mask_change_kernel<false, true><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
+        else if (h->aa && (h->t & 1) == 0)
             mask_change_kernel<true><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
         else
             mask_change_kernel<false><<<blocks, 256, 0, h->stream>>>(p, arr, p.solid, newm);
@@ -698,7 +701,8 @@ static cudaError_t launch_init_v(lbm_s *h, const KParams &p, int planes)
 {
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
     if (h->mask) {
-        if (h->aa) init_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p);
+        if (h->aax) init_kernel<V, WR_XO, true><<<grid, block, 0, h->stream>>>(p);
+        else if (h->aa) init_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p);
         else init_kernel<V, WR_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
     } else if (h->aax) init_kernel<V, WR_XO><<<grid, block, 0, h->stream>>>(p);
     else if (h->aa) init_kernel<V, WR_PUSH><<<grid, block, 0, h->stream>>>(p);
@@ -721,6 +725,8 @@ static cudaError_t launch_macros_v(lbm_s *h, const KParams &p, int planes)
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)planes * h->ny / h->TY * h->nchunk));
     if (h->mask) {
         if (!h->aa) macros_kernel<V, RD_PULL, true><<<grid, block, 0, h->stream>>>(p);
+        else if (h->aax && (h->t & 1) == 0) macros_kernel<V, RD_XE, true><<<grid, block, 0, h->stream>>>(p);
+        else if (h->aax) macros_kernel<V, RD_XO, true><<<grid, block, 0, h->stream>>>(p);
         else if ((h->t & 1) == 0) macros_kernel<V, RD_LOCAL, true><<<grid, block, 0, h->stream>>>(p);
         else macros_kernel<V, RD_PULL_OPP, true><<<grid, block, 0, h->stream>>>(p);
     } else if (!h->aa) macros_kernel<V, RD_PULL><<<grid, block, 0, h->stream>>>(p);
@@ -1397,6 +1403,8 @@ static cudaError_t launch_setstate_v(lbm_s *h, const KParams &p, const float *in
     dim3 block(h->TX, h->TY), grid((unsigned)((long long)h->nz * h->ny / h->TY * h->nchunk));
     if (h->mask) {
         if (!h->aa) setstate_kernel<V, WR_LOCAL, true><<<grid, block, 0, h->stream>>>(p, in);
+        else if (h->aax && odd) setstate_kernel<V, WR_XE, true><<<grid, block, 0, h->stream>>>(p, in);
+        else if (h->aax) setstate_kernel<V, WR_XO, true><<<grid, block, 0, h->stream>>>(p, in);
         else if (odd) setstate_kernel<V, WR_LOCAL_OPP, true><<<grid, block, 0, h->stream>>>(p, in);
         else setstate_kernel<V, WR_PUSH, true><<<grid, block, 0, h->stream>>>(p, in);
     } else if (!h->aa) setstate_kernel<V, WR_LOCAL><<<grid, block, 0, h->stream>>>(p, in);

@@ -88,6 +88,7 @@ struct KParams {
                                 // standard Smagorinsky model with the constants above (lbm_set_sgs_rows)
     const float *jref;          // [ny] r_j = J0_j / 12: per-row momentum reference (see mom_ref_shift)
     int bot, top, drag_vector;
+    int aax;                    // 1 = x-balanced AA storage (host-side kernels that address single entries)
     const unsigned *solid;      // per-cell solid bit mask, one word per 32 x cells (NULL = none)
     const unsigned *solid_nb;   // the same mask dilated by one cell in x, y, z (host-built)
     int nxw;                    // words per x row, ceil(nx / 32) (bits past nx in the last word are 0)
@@ -540,8 +541,12 @@ template <int V, int RM>
 __device__ __forceinline__ void solid_fix_loads(const KParams &p, const Ctx &c, float (&g)[Q][V],
                                                 unsigned long long S)
 {
-    if constexpr (RM == RD_LOCAL) return;
-    static_assert(RM == RD_LOCAL || RM == RD_PULL || RM == RD_PULL_OPP, "the geometry variants exist for two-lattice and AA storage");
+    // RD_LOCAL / RD_XE (the even steps of the single-array schemes): every population waits where the
+    // odd step - which knows the geometry - has put it; nothing to correct.
+    if constexpr (RM == RD_LOCAL || RM == RD_XE) return;
+    // x-balanced AA, odd step: a bounce changes slot and row only, the x displacement of the fetch stays
+    // (c_x = +1 populations come from x - 1 of the own row as well)
+    constexpr bool AAX = (RM == RD_XO);
     // Which cells of direction i bounce: the bits of the source cells x0+k - c_x in the row load_dir used.
     auto bounce_bits = [&](auto ic) -> unsigned {
         constexpr int i = decltype(ic)::value;
@@ -563,7 +568,14 @@ __device__ __forceinline__ void solid_fix_loads(const KParams &p, const Ctx &c, 
             constexpr int j = decltype(jc)::value, i = i0 + j;
             constexpr int S_BB = (RM == RD_PULL) ? Lat::opp[i] : i;
             bits[j] = bounce_bits(std::integral_constant<int, i>{});
-            if (bits[j]) ldv<V>(ownp + (long long)S_BB * p.N, own[j]);
+            if constexpr (AAX && Lat::cx[i] == 1) {
+                const float *q = ownp + (long long)S_BB * p.N;
+#pragma unroll
+                for (int k = 0; k < V; ++k)
+                    if ((bits[j] >> k) & 1u) own[j][k] = (k == 0) ? q[c.xl - c.x0] : q[k - 1];
+            } else {
+                if (bits[j]) ldv<V>(ownp + (long long)S_BB * p.N, own[j]);
+            }
         });
         static_for<0, 6>([&](auto jc) {
             constexpr int j = decltype(jc)::value, i = i0 + j;
@@ -585,8 +597,7 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float 
             constexpr int i = decltype(ic)::value;
             store_dir<V, WM, i>(p, c, g[i]);
         });
-    } else if constexpr (WM != WR_PUSH) {
-        static_assert(WM == WR_LOCAL || WM == WR_LOCAL_OPP, "the geometry variants exist for two-lattice and AA storage");
+    } else if constexpr (WM != WR_PUSH && WM != WR_XO) {
         const unsigned self = solid_self<V>(S);
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
@@ -596,11 +607,16 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float 
             store_dir<V, WM, i>(p, c, g[i]);
         });
     } else {
+        // WR_PUSH (AA) and WR_XO (x-balanced AA): the odd steps.  In the x-balanced pattern the values of
+        // a c_x = -1 direction land one cell to the left and nothing else moves in x, whether the link
+        // is open or bounces (a bounce changes slot and row only).
+        constexpr bool AAX = (WM == WR_XO);
         const unsigned selff = solid_pick(S, 1, 1), self = solid_self<V>(S);
         const long long own = (long long)(c.y + p.ny * c.z) * p.nx + c.x0;
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int cx = Lat::cx[i], cy = Lat::cy[i], cz = Lat::cz[i];
+            constexpr int XS = AAX ? (cx == -1 ? -1 : 0) : cx;      // x displacement of the stored values
             bool bb = false, fs = false;
             if constexpr (cy == -1) bb = c.bot_bb;
             if constexpr (cy == 1) { bb = c.top_bb; fs = c.top_fs; }
@@ -612,8 +628,8 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float 
             store_dir<V, WM, i>(p, c, g[i], fast);
             // the element a vector-path x neighbour expects THIS lane to store for it
             float nb = 0.f;
-            if constexpr (V > 1 && cx == 1) nb = __shfl_up_sync(0xffffffffu, g[i][V - 1], 1);
-            if constexpr (V > 1 && cx == -1) nb = __shfl_down_sync(0xffffffffu, g[i][0], 1);
+            if constexpr (V > 1 && XS == 1) nb = __shfl_up_sync(0xffffffffu, g[i][V - 1], 1);
+            if constexpr (V > 1 && XS == -1) nb = __shfl_down_sync(0xffffffffu, g[i][0], 1);
             if (!fast) {
                 const int ysel = (cy == 0) ? c.y : (cy == 1 ? c.yp : c.ym);
                 const int zsel = (cz == 0) ? c.z : (cz == 1 ? c.zp : c.zm);
@@ -622,6 +638,24 @@ __device__ __forceinline__ void store_all(const KParams &p, const Ctx &c, float 
                 const int yrow = fs ? c.y : ysel;
                 float *rowp = p.dst + (long long)slot * p.N + (long long)(yrow + p.ny * zsel) * p.nx;
                 float *ownp = p.dst + (long long)S_OPP * p.N + own;
+                if constexpr (AAX) {
+                    float *ownrow = ownp - c.x0;                          // slot opp(i), own row
+#pragma unroll
+                    for (int k = 0; k < V; ++k) {
+                        if ((self >> k) & 1u) continue;                   // solid source: nothing leaves it
+                        int xd = c.x0 + k + XS;
+                        xd = (xd < 0) ? p.nx - 1 : xd;
+                        const bool bounced = bb || ((destf >> (k + cx + 1)) & 1u);
+                        (bounced ? ownrow : rowp)[xd] = g[i][k];
+                    }
+                    // the element a vector-path right neighbour expects THIS lane to store for it (its
+                    // cell x0+V, landing on x0+V-1), bounced or not
+                    if constexpr (V > 1 && XS == -1) {
+                        if (!c.edgeR && !((selff >> (V + 1)) & 1u))
+                            ((bb || ((destf >> V) & 1u)) ? ownrow : rowp)[c.x0 + V - 1] = nb;
+                    }
+                    return;
+                }
 #pragma unroll
                 for (int k = 0; k < V; ++k) {
                     if ((self >> k) & 1u) continue;                       // solid source: nothing leaves it
@@ -1252,7 +1286,14 @@ __device__ __forceinline__ bool mask_bit(const unsigned *mask, const KParams &p,
 //                           and n's slot receives d's rest population (0);
 //            d turns solid: n's population that had entered d bounces instead (moves to the own
 //                           slot of n, replacing what d had pushed there); d is cleared.
-template <bool PUSH>
+//   AAX (x-balanced AA, either parity): the same, with every slot whose c_x is +1 kept one cell to the
+//          left of the cell it belongs to (slot s of cell n sits at n - [c_sx = +1] e_x).
+__device__ __forceinline__ long long left_of(const KParams &p, long long cell, bool shift)
+{
+    if (!shift) return cell;
+    return (cell % p.nx == 0) ? cell + p.nx - 1 : cell - 1;
+}
+template <bool PUSH, bool AAX = false>
 __global__ void mask_change_kernel(const KParams p, float *arr, const unsigned *oldm, const unsigned *newm)
 {
     const long long d = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1269,8 +1310,11 @@ __global__ void mask_change_kernel(const KParams p, float *arr, const unsigned *
             const PushLoc t = push_target<i>(p, is ? oldm : newm, x, y, z);
             if (t.self) return;
             if (mask_bit(oldm, p, t.cell) || mask_bit(newm, p, t.cell)) return;   // n must be fluid before and after
-            float *at_n = arr + (long long)t.slot * p.N + t.cell;          // n's own slot on this link
-            float *at_d = arr + (long long)Lat::opp[i] * p.N + d;          // where n's population enters d
+            // n's own slot on this link (slot i, or its y mirror at a free-slip face: the same c_x)
+            constexpr bool sh_n = AAX && Lat::cx[i] == 1, sh_d = AAX && Lat::cx[i] == -1;
+            float *at_n = arr + (long long)t.slot * p.N + left_of(p, t.cell, sh_n);
+            // where n's population enters d (slot opp(i))
+            float *at_d = arr + (long long)Lat::opp[i] * p.N + left_of(p, d, sh_d);
             if (!is) { *at_d = *at_n; *at_n = 0.f; }                        // d turns fluid
             else *at_n = *at_d;                                             // d turns solid
         });
@@ -1278,7 +1322,8 @@ __global__ void mask_change_kernel(const KParams p, float *arr, const unsigned *
     if (is) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            arr[(long long)i * p.N + d] = 0.f;
+            constexpr bool sh = AAX && Lat::cx[i] == 1;
+            arr[(long long)i * p.N + left_of(p, d, sh)] = 0.f;
         });
     }
 }
@@ -1315,6 +1360,8 @@ __global__ void state_kernel(const KParams p, float *out)
             v = p.src[(long long)S_OPP * p.N + (cell - x + xd)];
         } else {
             int slot = i, xd = x + (MODE == 4 ? xdx : cx), yd = y + cy, zd = z + cz;
+            int xt = x + cx;                                   // the cell the link leads to
+            xt = (xt < 0) ? p.nx - 1 : (xt >= p.nx ? 0 : xt);
             xd = (xd < 0) ? p.nx - 1 : (xd >= p.nx ? 0 : xd);
             zd = (zd < 0) ? p.nz - 1 : (zd >= p.nz ? 0 : zd);
             if (yd < 0) {
@@ -1326,6 +1373,8 @@ __global__ void state_kernel(const KParams p, float *out)
                 else { slot = S_OPP; xd = (MODE == 4) ? xd : x; yd = y; zd = z; }
             }
             if (MODE == 2 && solid_at(p, xd, yd, zd)) { slot = S_OPP; xd = x; yd = y; zd = z; }
+            // x-balanced: a link that bounces off a solid changes slot and row, not the x displacement
+            if (MODE == 4 && solid_at(p, xt, yd, zd)) { slot = S_OPP; yd = y; zd = z; }
             v = p.src[(long long)slot * p.N + ((long long)(yd + p.ny * zd) * p.nx + xd)];
         }
         out[(long long)i * p.N + cell] = self_solid ? 0.f : v;
@@ -1407,10 +1456,13 @@ __global__ void halo_kernel(const KParams p, float *pops, HaloFace f0, HaloFace 
             else if (p.top == BC_TOP_SLIP) ys = y;                          // mirrored link from the same row
             else return;
         }
-        int xs = x - cxs[i];
+        // x-balanced AA: the entry at memory column x belongs to cell x + 1 when c_x = +1
+        int xc = x + ((p.aax && cxs[i] == 1) ? 1 : 0);
+        xc = (xc >= p.nx) ? 0 : xc;
+        int xs = xc - cxs[i];
         xs = (xs < 0) ? p.nx - 1 : (xs >= p.nx ? 0 : xs);
         const int zs = side ? z - 1 : z + 1;                                 // the ghost plane it came from
-        if (p.solid && (solid_at(p, x, y, z) || solid_at(p, xs, ys, zs))) return;
+        if (p.solid && (solid_at(p, xc, y, z) || solid_at(p, xs, ys, zs))) return;
     }
     float *cell = pops + (long long)i * p.N + (long long)z * plane + r;
     if (PACK) buf[q] = *cell; else *cell = buf[q];

@@ -1,6 +1,6 @@
 // lbm_step_inst.cu — one explicit instantiation of the step-kernel launcher, selected by
 // -DLBM_V=<1|2|4> -DLBM_S=<0|1> -DLBM_G=<0|1> (cells per thread, fused statistics, row-table SGS):
-// 8 kernels per translation unit (5 storage modes + 3 geometry variants).  build.py compiles the
+// 10 kernels per translation unit (5 storage modes, each also as a geometry variant).  build.py compiles the
 // twelve of them in parallel.
 #include "lbm_launch.cuh"
 
@@ -22,6 +22,8 @@ cudaError_t launch_step_t(const StepLaunch &L, const KParams &p0)
     cudaStream_t st = L.stream;
     if (L.mask) {
         if (!L.aa) return launch_chain(step_kernel<V, RD_PULL, WR_LOCAL, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
+        else if (L.aax && !L.odd) return launch_chain(step_kernel<V, RD_XE, WR_XE, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
+        else if (L.aax) return launch_chain(step_kernel<V, RD_XO, WR_XO, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
         else if (!L.odd) return launch_chain(step_kernel<V, RD_LOCAL, WR_LOCAL_OPP, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
         else return launch_chain(step_kernel<V, RD_PULL_OPP, WR_PUSH, STATS, true, SGS>, grid, block, 0, st, L.pdl, p);
     } else if (!L.aa) return launch_chain(step_kernel<V, RD_PULL, WR_LOCAL, STATS, false, SGS>, grid, block, 0, st, L.pdl, p);

@@ -457,13 +457,14 @@ def _solid_mask(kind, nx, ny, nz):
     return m
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("kind", ["random", "boxes", "top"])
 @pytest.mark.parametrize("nx,vec", [(64, 4), (96, 4), (64, 2), (32, 1)])
 def test_solid_mask_parity(orc, gpu, aa, kind, nx, vec):
     cfg = wl.small(nx=nx, ny=10, nz=6)
     cfg["solid"] = _solid_mask(kind, nx, 10, 6)
     o, g = _pair(orc, gpu, cfg, aa, vec)
+    assert g.variant.startswith({False: "pull2/", True: "aa/", "aax": "aax/"}[aa])
     w = _weights(orc)
     assert _state_err(o, g, w) <= 5e-8
     o.stats_accumulate(1)
@@ -485,7 +486,7 @@ def test_solid_mask_parity(orc, gpu, aa, kind, nx, vec):
     assert np.all(rg.cpu().numpy()[solid] == 1.0) and np.all(ug.cpu().numpy()[:, solid] == 0.0)
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("nx,vec", [(36, 4), (70, 2), (33, 1), (100, 4)])
 def test_solid_mask_on_ragged_rows(orc, gpu, aa, nx, vec):
     """nx not a multiple of 32: the mask rows are padded to whole words (the paper's own meshes are
@@ -503,7 +504,7 @@ def test_solid_mask_on_ragged_rows(orc, gpu, aa, nx, vec):
         assert _state_err(o, g, w) <= 2e-7
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("t_change", [6, 7])
 @pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2)])
 def test_solid_removed_at_run_time_keeps_the_flow(orc, gpu, aa, t_change, nx, vec):
@@ -537,7 +538,7 @@ def test_solid_removed_at_run_time_keeps_the_flow(orc, gpu, aa, t_change, nx, ve
     assert float(ug[0].cpu().numpy()[boxes].std()) > 1e-4
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 @pytest.mark.parametrize("nx,vec", [(64, 4), (36, 4), (34, 2), (33, 1)])
 def test_forest_codes_parity(orc, gpu, aa, nx, vec):
     """Per-cell forest codes: a forest edge in x, a clearing in z, two canopy
@@ -617,8 +618,6 @@ def test_graph_replay_is_bit_identical(gpu, aa, every):
 @pytest.mark.parametrize("nx", [64, 36, 33])
 def test_sweep_direction_is_bit_identical(gpu, aa, solid, nx):
     import torch
-    if aa == "aax" and solid:
-        pytest.skip("the x-balanced AA storage has no geometry variant")
     cfg = wl.small(nx=nx, ny=12, nz=10)
     if solid:
         m = np.zeros((cfg["nz"], cfg["ny"], cfg["nx"]), dtype=np.uint8)
@@ -664,8 +663,6 @@ _GUARD_SHAPES = [(64, 12, 10, 4), (36, 7, 5, 4), (34, 5, 3, 2), (33, 3, 4, 1), (
 @pytest.mark.parametrize("kind", ["plain", "solid", "slab"])
 def test_guard_bands_stay_untouched(gpu, aa, kind):
     import torch
-    if kind == "solid" and aa == "aax":
-        pytest.skip("the x-balanced AA storage has no geometry variant")
     for nx, ny, nz, vec in _GUARD_SHAPES:
         if kind == "slab" and nz < 3:
             continue
@@ -708,7 +705,7 @@ def test_guard_bands_stay_untouched(gpu, aa, kind):
             g.close()
 
 
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 def test_masked_update_is_run_to_run_bit_identical(gpu, aa):
     """Five runs of a lattice with 15 % random solids (every lane takes the element-store path
     somewhere) and of a plain one: identical to the last bit."""
@@ -752,8 +749,6 @@ def test_step_before_init_is_an_error(gpu):
 @pytest.mark.parametrize("t0", [4, 7])
 @pytest.mark.parametrize("solid", [False, True])
 def test_get_state_set_state_round_trip_is_bit_identical(gpu, aa, t0, solid):
-    if aa == "aax" and solid:
-        pytest.skip("the x-balanced AA storage has no geometry variant")
     """get_state -> set_state(t) into a fresh handle -> step continues the run bit for bit."""
     import torch
     cfg = wl.small(nx=64, ny=10, nz=6)

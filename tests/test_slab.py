@@ -88,8 +88,6 @@ def test_emulated_slabs_equal_global_lattice(world, case, storage):
     import paper_2206_15454_b200 as lb
     from paper_2206_15454_b200 import slab
 
-    if storage == "aax" and "solid" in case:
-        pytest.skip("the x-balanced AA storage has no geometry variant")
     cfg = wl.small(nx=32, ny=10, nz=12)
     if case == "periodic":
         cfg = wl.small(nx=32, ny=10, nz=12, bottom=wl.PERIODIC, top=wl.PERIODIC)
