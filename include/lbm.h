@@ -113,7 +113,13 @@ int lbm_set_top_velocity(lbm_t *h, const double *U_top);
  * computational domain.  The flow remains in the turbulent status afterwards") - every cell that
  * stays fluid keeps its populations bit for bit, a cell that turns fluid starts at rest
  * (f = f_eq(1, 0), reading R28), a cell that turns solid is cleared; lbm_time is unchanged.
- * Synchronises the stream.
+ * Synchronises the stream.  On a z slab (LBM_Z_HALO) the mask covers the two ghost planes as well
+ * and every rank changes its mask at the same time step; after a change on a running handle the
+ * caller repeats the halo exchange (lbm_halo_pack, exchange, lbm_halo_unpack on both faces) before
+ * the next step: in the single-array storages at even time steps the populations that move
+ * between a changed cell and a neighbour across a slab face are converted in the ghost planes of
+ * the rank that holds them and travel with that exchange (at odd steps and in two-lattice storage
+ * the exchange repeats what the planes already hold).
  *
  * lbm_set_forest_codes: heterogeneous canopies (L129-135: "The code for each forest cell contains
  * ... h ... y ... y_m ... stored into the forest cell's code using a bit mask"; Alg. 1 "if

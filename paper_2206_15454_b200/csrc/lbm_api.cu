@@ -521,9 +521,9 @@ int lbm_set_solid(lbm_t *h, const uint8_t *solid_host)
     DevGuard dg(h);
     if (!h->mask) return fail(LBM_EINVAL, "handle was not created with LBM_SOLID_MASK");
     if (!h->bound) return fail(LBM_ESTATE, "lbm_set_solid before lbm_bind");
-    if (h->inited && h->halo && h->aa && (h->t & 1) == 0)
-        return fail(LBM_ESTATE, "on a single-array z slab a running mask change needs an odd time step "
-                                "(at even t populations of the neighbour slabs sit in this slab's planes)");
+    // (z slab, single-array storage, even t: populations that cross a slab face sit in the ghost planes of
+    // the rank that pushed them; the conversion below works on every local plane, ghosts included, and
+    // the caller then repeats the halo exchange - lbm.h)
     const int nxw = (h->nx + 31) / 32;
     const size_t words = (size_t)nxw * h->ny * h->nz;
     std::vector<uint32_t> bits;

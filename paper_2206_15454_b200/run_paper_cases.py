@@ -79,7 +79,7 @@ def run_case(lb, cfg: dict, spinup: int, window: int, boxes: bool, device="cuda:
     c = dict(cfg)
     if boxes:
         c["geometry"] = True
-    sim = lb.Lbm.from_config(c, aa=True if boxes else "aax", device=device)   # geometry handles: plain AA
+    sim = lb.Lbm.from_config(c, aa="aax", device=device)    # single array, x-balanced AA (geometry handles too)
     if boxes:
         sim.set_solid(trip_boxes(cfg))
     sim.init(cfg["seed"])

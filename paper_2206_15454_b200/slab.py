@@ -61,6 +61,7 @@ class SlabLbm:
             raise ValueError(f"nz={cfg['nz']} is not a multiple of the number of slabs {world}")
         self.rank, self.world, self.group = int(rank), int(world), group
         self.emulated = bool(emulated)      # the caller drives the exchange (exchange_emulated)
+        self._inited = False                # a state exists (init / set_macros): halo calls are allowed
         self.nz_global = cfg["nz"]
         self.nz_local = cfg["nz"] // world
         self.z_first = self.rank * self.nz_local
@@ -108,12 +109,29 @@ class SlabLbm:
     # -- the Lbm calls, slab-aware -----------------------------------------------------------
     def init(self, seed: int):
         self.sim.init(seed)
+        self._inited = True
         self.exchange()
 
     def set_macros(self, rho_local, u_local):
         """Fields of the local planes INCLUDING the two ghost planes (nz_local + 2)."""
         self.sim.set_macros(rho_local, u_local)
+        self._inited = True
         self.exchange()
+
+    def _local_mask(self, solid_global):
+        """The slab's planes of a global [nz][ny][nx] mask, the two ghost planes included."""
+        if solid_global is None:
+            return None
+        z = np.arange(self.z_first - 1, self.z_first + self.nz_local + 1) % self.nz_global
+        return np.ascontiguousarray(np.asarray(solid_global)[z])
+
+    def set_solid(self, solid_global):
+        """Change the solid mask (GLOBAL [nz][ny][nx], None = no solid cell) on every rank at the same
+        time step; on a running slab the flow is kept and the halo exchange is repeated
+        (lbm.h: lbm_set_solid on a z slab)."""
+        self.sim.set_solid(self._local_mask(solid_global))
+        if self._inited:
+            self.exchange()
 
     def stats_accumulate(self, every: int = 1):
         self.sim.stats_accumulate(every)
@@ -206,6 +224,14 @@ def init_emulated(slabs, seed: int):
     for s in slabs:
         s.init(seed)
     exchange_emulated(slabs)
+
+
+def set_solid_emulated(slabs, solid_global):
+    """SlabLbm.set_solid for a ring of emulated slabs: every slab changes its mask, then one exchange."""
+    for s in slabs:
+        s.sim.set_solid(s._local_mask(solid_global))
+    if slabs[0]._inited:
+        exchange_emulated(slabs)
 
 
 def exchange_emulated(slabs):

@@ -61,7 +61,7 @@ def test_oracle_shows_what_the_text_says(orc, oracle_cases):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("aa", [False, True], ids=["pull2", "aa"])
+@pytest.mark.parametrize("aa", [False, True, "aax"], ids=["pull2", "aa", "aax"])
 def test_gpu_cases_agree_with_the_oracle(orc, oracle_cases, aa):
     import torch
     if not torch.cuda.is_available():
@@ -109,3 +109,22 @@ def test_runner_with_row_table_sgs_models(sgs):
         stats[k] = st
     ck = text_checks(stats, 7)
     assert ck["case3_gradient_largest"] and ck["case3_near_ground_u_largest"] and ck["cases_1_2_differ_slightly"]
+
+
+@pytest.mark.gpu
+def test_runner_with_trip_boxes_removed_at_run_time():
+    """run_paper_cases.run_case(boxes=True): the paper's spin-up method (L226) on the oracle-sized ABL -
+    trip boxes in place during the spin-up, removed on the running handle, statistics afterwards.
+    The boxes must have perturbed the flow (the mean profile differs from the run without them) and
+    the result stays a sane canopy flow."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200.run_paper_cases import run_case
+    cfg = wl.abl_case_small(1)
+    st_b, us_b, mlups = run_case(lb, cfg, SPINUP, WINDOW, boxes=True)
+    st_p, us_p, _ = run_case(lb, cfg, SPINUP, WINDOW, boxes=False)
+    assert np.isfinite(st_b).all() and mlups > 0 and us_b > 0 and us_p > 0
+    assert np.abs(st_b[:, 0] - st_p[:, 0]).max() > 1e-4 * cfg["u_bulk"]
+    assert np.all(st_b[:, 0] > -0.2 * cfg["u_bulk"]) and st_b[-1, 0] > st_b[0, 0]

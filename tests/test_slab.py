@@ -253,3 +253,52 @@ def test_single_slab_overlapped_through_the_comm_stream(storage):
     torch.cuda.synchronize()
     assert torch.equal(a.get_macros()[1], ref.get_macros()[1])
     assert torch.equal(b.get_macros()[1], ref.get_macros()[1])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("storage", ["two_lattice", "aa", "aax"])
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("t_change", [4, 5])
+def test_solid_removed_at_run_time_on_slabs(world, storage, t_change):
+    """PAPER.md:L226 on a cut lattice: boxes across slab faces are removed (and others put in) on
+    running slabs at an even and at an odd time step; the ring must go on like the undivided lattice.
+    In the single-array storages at even t the populations between a changed cell and a neighbour
+    across a face are converted in the ghost planes and travel with the repeated exchange."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2206_15454_b200 as lb
+    from paper_2206_15454_b200 import slab
+
+    cfg = wl.small(nx=32, ny=10, nz=12)
+    m = np.zeros((12, 10, 32), bool)
+    m[0:2, 0:3, 4:9] = True                          # straddles the z wrap ...
+    m[11, 0:3, 4:9] = True
+    m[3:9, 2:5, 30:] = True                          # ... crosses the slab faces of 2 and 3 slabs and the x wrap
+    m[3:9, 2:5, :2] = True
+    cfg["solid"] = m
+    moved = np.zeros_like(m)
+    moved[5:10, 4:8, 10:14] = True                   # new solids across other faces, the old ones gone
+    moved[0, 0:2, 20:24] = True
+    aa = {"two_lattice": False, "aa": True, "aax": "aax"}[storage]
+    ref = lb.Lbm.from_config(cfg, aa=aa, vec=4)
+    ref.init(cfg["seed"])
+    slabs = [slab.SlabLbm(cfg, r, world, emulated=True, storage=storage, vec=4) for r in range(world)]
+    slab.init_emulated(slabs, cfg["seed"])
+    ref.step(t_change)
+    slab.step_emulated(slabs, t_change)
+    part = m.copy()
+    part[3:9, 2:5, 30:] = False
+    for mask, n in ((part, 3), (None, 2), (moved, 3), (None, 6)):
+        ref.set_solid(mask)
+        slab.set_solid_emulated(slabs, mask)
+        for k in range(n):
+            ref.step(1)
+            slab.step_emulated(slabs, 1, overlap=bool(k & 1))
+            rr, ur = ref.get_macros()
+            rs = torch.cat([s.get_macros()[0] for s in slabs], dim=0)
+            us = torch.cat([s.get_macros()[1] for s in slabs], dim=1)
+            assert float((rs - rr).abs().max()) <= 2e-7 and float((us - ur).abs().max()) <= 5e-8, (mask is None, k)
+    for s in slabs:
+        s.close()
+    ref.close()
