@@ -3,7 +3,7 @@
 The shared object is built in-tree (git-ignored) so that it travels to the GPU box with the
 repository snapshot.  `python -m paper_2206_15454_b200.build [--force] [--verbose]`.
 
-The step kernel exists in ~110 variants (cells per thread x storage mode x statistics x geometry x
+The step kernel exists in ~130 variants (cells per thread x storage mode x statistics x geometry x
 SGS table, plus the TMA tiles); they are spread over 15 translation units (csrc/lbm_step_inst.cu and
 csrc/lbm_tma_inst.cu compiled once per template-argument set) that compile in parallel, then one link.
 """

@@ -1,5 +1,5 @@
 // lbm_launch.cuh — launchers of the fused step kernel, one explicit instantiation per translation
-// unit so that the ~110 step-kernel variants compile in parallel (build.py).
+// unit so that the ~130 step-kernel variants compile in parallel (build.py).
 //
 // lbm_api.cu fills a StepLaunch (the few handle fields a launch needs) and calls
 // launch_step_t<V, STATS, SGS> / launch_tma_t<STATS>; lbm_step_inst.cu and lbm_tma_inst.cu hold the
