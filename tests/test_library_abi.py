@@ -190,3 +190,31 @@ def test_sgs_row_table_helpers_closed_forms(lb):
     assert np.isclose(S[0], 0.5 * (st[0, 0] + st[1, 0]) * np.sqrt(1.25), rtol=1e-13) and np.isclose(S[-1], S[0], rtol=1e-12)
     S2 = lb.sgs_mean_shear(st, top_wall=False)
     assert np.isclose(S2[-1], 0.5 * abs(st[-1, 0] - st[-2, 0]) * np.sqrt(1.25), rtol=1e-12)
+
+
+def test_block_shapes_of_the_configs_and_the_paper_meshes(lb):
+    """Host logic of lbm_create (no GPU): cells per thread and thread-block shape per lattice width.
+    Whole-warp row segments where the width offers them; the paper's meshes (PAPER.md:L171, L244:
+    372, 350, 250, 200 cells wide) take one irregular row segment per block; lattices of <= 2^17
+    cells run one cell per thread; the x-balanced storage accepts geometry handles."""
+    L = lb.lib()
+    L.lbm_variant.restype = C.c_char_p
+    bf = (C.c_double * 3)(0, 0, 0)
+    dp = C.POINTER(C.c_double)
+    cases = [
+        ((1536, 384, 1024), lb.STORAGE_AAX, "aax/v4/tx128x1"),
+        ((1024, 256, 512), lb.STORAGE_AAX | lb.SOLID_MASK, "aax/v4/tx128x1"),
+        ((512, 128, 256), 0, "pull2/v4/tx128x1"),
+        ((64, 32, 32), 0, "pull2/v1/tx64x2"),
+        ((372, 62, 124), 0, "pull2/v4/tx93x1"),
+        ((350, 140, 280), lb.STORAGE_AAX, "aax/v2/tx175x1"),
+        ((250, 100, 200), lb.STORAGE_AA, "aa/v2/tx125x1"),
+        ((200, 80, 160), 0, "pull2/v4/tx50x1"),
+    ]
+    for (nx, ny, nz), flags, want in cases:
+        h = C.c_void_p()
+        rc = L.lbm_create(C.byref(h), nx, ny, nz, 1e-4, 0.1, C.cast(bf, dp), 0.0, None, flags | lb.TOP_FREE_SLIP)
+        assert rc == 0, (nx, ny, nz, L.lbm_last_error())
+        got = L.lbm_variant(h).decode()
+        L.lbm_destroy(h)
+        assert got == want, ((nx, ny, nz), got, want)
