@@ -191,11 +191,11 @@ __device__ __forceinline__ void block_index3(const KParams &p, int &cb, int &yb,
 // index of the block in the whole-lattice order of the 1-D launch (per-block geometry flags)
 __device__ __forceinline__ long long block_linear(const KParams &p)
 {
-    const int rows_per_plane = p.ny / (int)blockDim.y;
     if (p.grid3) {
+        // gridDim.y is the number of row blocks of a plane: no division on this path
         int cb, yb, zb;
         block_index3(p, cb, yb, zb);
-        return ((long long)(p.z0 + zb) * rows_per_plane + yb) * p.nchunk + cb;
+        return ((long long)(p.z0 + zb) * (int)gridDim.y + yb) * p.nchunk + cb;
     }
     return (long long)block_index(p) + (long long)(p.z0 * p.ny / (int)blockDim.y) * p.nchunk;
 }
